@@ -177,6 +177,9 @@ int orc_sweep_y(double* f, int nx, int ny, int g, const int* nv, const double* v
     const long S = G.nvtot;
     const long rowstride = (long)nx * S;
     int err = ERR_OK;
+    // eq. (38): every flux is taken from the OLD f.  A REFLECT side reads the line with v_y mirrored, which
+    // is another line of the same array, so the sweep reads from a snapshot and writes into f.
+    const std::vector<double> old(f, f + (long)G.nyg * rowstride);
 #pragma omp parallel
     {
         std::vector<double> out(ny), sig(ny + 1);
@@ -194,16 +197,16 @@ int orc_sweep_y(double* f, int nx, int ny, int g, const int* nv, const double* v
                             if (bc_lo == BC_PERIODIC) r += ny;
                             else if (bc_lo == BC_REFLECT) { r = -1 - r; vv = (vv == v) ? vmir : v; }
                             else { if (r + g < 0) { lerr = ERR_SHIFT; return 0.0; }
-                                   return f[(r + g) * rowstride + (long)ix * S + vv]; }
+                                   return old[(r + g) * rowstride + (long)ix * S + vv]; }
                         } else {
                             if (bc_hi == BC_PERIODIC) r -= ny;
                             else if (bc_hi == BC_REFLECT) { r = 2L * ny - 1 - r; vv = (vv == v) ? vmir : v; }
                             else { if (r + g >= G.nyg) { lerr = ERR_SHIFT; return 0.0; }
-                                   return f[(r + g) * rowstride + (long)ix * S + vv]; }
+                                   return old[(r + g) * rowstride + (long)ix * S + vv]; }
                         }
                     }
                     if (r < 0 || r >= ny) { lerr = ERR_SHIFT; return 0.0; }
-                    return f[(r + g) * rowstride + (long)ix * S + vv];
+                    return old[(r + g) * rowstride + (long)ix * S + vv];
                 };
                 std::vector<double> phi(ny + 1);
                 for (int k = 0; k <= ny; ++k) phi[k] = pfc_flux(get, k - 1, s, finf, limiter);

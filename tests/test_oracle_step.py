@@ -1,0 +1,234 @@
+"""Pins for the oracle's spatial sweeps and full step: T10 (free streaming = exact translation at integer
+shifts), T11 (uniform Maxwellian invariant bit-for-bit), T5 (mass to round-off over a full step), the
+y-boundary kinds (method of images for REFLECT, Dirichlet ghost rows for FLUID, R9 shift bound), T16
+(second order of the Strang splitting) and T12 (linear Landau damping rate at k = 0.5).
+None of them re-types the oracle's formulas."""
+import numpy as np
+import pytest
+
+from paper_1406_5445_b200 import inputs
+
+
+def _species(orc, nv, vmin, vmax, q=-1.0, m=1.0, finf=1.0):
+    return orc.Species(q, m, nv, vmin, vmax, finf)
+
+
+def test_T10_free_streaming_is_exact_translation(orc):
+    # v centres -3,-1,1,3 (x), -2.5,-1.5,...(y scaled so shifts are integers): dt/(2 dx) = 1, dt/(2 dy) = 2
+    nx, ny = 12, 10
+    nv = (4, 4, 2)
+    sp = _species(orc, nv, (-4.0, -1.0, -1.0), (4.0, 1.0, 1.0))
+    lx, ly, dt = 12.0, 2.5, 2.0          # dx = 1, dy = 0.25: sx = vx*1, sy = vy*dt/(2dy) = vy*4 -> vy=+-0.25,+-0.75 -> +-1,+-3
+    rng = np.random.default_rng(10)
+    f0 = rng.random((ny, nx) + nv)
+    f = f0.copy()
+    Z = np.zeros((3, ny, nx))
+    err, _ = orc.step(f, sp, nx, ny, 0, lx, ly, dt, Z, Z, limiter=1)
+    assert err == 0
+    vx = sp.vmin[0] + (np.arange(nv[0]) + 0.5) * 2.0
+    vy = sp.vmin[1] + (np.arange(nv[1]) + 0.5) * 0.5
+    for a in range(nv[0]):
+        for b in range(nv[1]):
+            sx = int(round(vx[a] * dt / (lx / nx)))
+            sy = int(round(vy[b] * dt / (ly / ny)))
+            assert sx != 0 and sy != 0
+            want = np.roll(f0[:, :, a, b, :], (sy, sx), axis=(0, 1))
+            assert np.abs(f[:, :, a, b, :] - want).max() <= 1e-14, (a, b)
+
+
+@pytest.mark.parametrize("bc", ["periodic", "reflect"])
+def test_T11_uniform_maxwellian_is_invariant_bit_for_bit(orc, bc):
+    nx, ny, nv = 6, 5, (8, 8, 8)
+    sp = _species(orc, nv, (-6.0,) * 3, (6.0,) * 3)
+    c = sp.vmin[0] + (np.arange(8) + 0.5) * 1.5
+    g = np.exp(-c ** 2 / 2) / np.sqrt(2 * np.pi)
+    M = g[:, None, None] * g[None, :, None] * g[None, None, :]
+    f0 = np.ascontiguousarray(np.broadcast_to(M, (ny, nx) + nv))
+    sp.f_inf = float(f0.max())
+    f = f0.copy()
+    Z = np.zeros((3, ny, nx))
+    b = orc.BC_PERIODIC if bc == "periodic" else orc.BC_REFLECT
+    err, mom = orc.step(f, sp, nx, ny, 0, 3.0, 2.0, 0.37, Z, Z, bc_lo=b, bc_hi=b)
+    assert err == 0
+    assert np.array_equal(f, f0)
+    assert np.ptp(mom[0]) == 0.0
+
+
+def _smooth_state(nx, ny, nv, sp, rng):
+    x = (np.arange(nx) + 0.5) / nx
+    y = (np.arange(ny) + 0.5) / ny
+    c = [sp.vmin[d] + (np.arange(nv[d]) + 0.5) * (sp.vmax[d] - sp.vmin[d]) / nv[d] for d in range(3)]
+    g = [np.exp(-(c[d] - 0.3 * d) ** 2 / 2) for d in range(3)]
+    M = g[0][:, None, None] * g[1][None, :, None] * g[2][None, None, :]
+    prof = 1 + 0.3 * np.cos(2 * np.pi * x)[None, :] * np.sin(2 * np.pi * y)[:, None] + 0.1 * rng.random((ny, nx))
+    return prof[:, :, None, None, None] * M[None, None]
+
+
+@pytest.mark.parametrize("bc", ["periodic", "reflect"])
+def test_T5_full_step_conserves_mass_to_roundoff(orc, bc):
+    nx, ny, nv = 8, 6, (8, 8, 8)
+    sp = _species(orc, nv, (-5.0,) * 3, (5.0,) * 3, q=-1.0, m=0.5)
+    rng = np.random.default_rng(5)
+    f = _smooth_state(nx, ny, nv, sp, rng)
+    sp.f_inf = float(f.max())
+    E = 0.5 * rng.normal(size=(3, ny, nx))
+    B = 0.5 * rng.normal(size=(3, ny, nx))
+    b = orc.BC_PERIODIC if bc == "periodic" else orc.BC_REFLECT
+    m0 = f.sum()
+    for _ in range(3):
+        err, mom = orc.step(f, sp, nx, ny, 0, 4.0, 3.0, 0.2, E, B, bc_lo=b, bc_hi=b)
+        assert err == 0
+    assert abs(f.sum() - m0) / m0 <= 1e-14
+    dv3 = (10.0 / 8) ** 3
+    assert abs(mom[0].sum() - f.sum() * dv3) <= 1e-13 * mom[0].sum()
+
+
+def test_y_sweep_periodic_equals_x_sweep_on_transposed_data(orc):
+    n, nv = 7, (4, 4, 3)
+    sp = _species(orc, nv, (-2.0, -2.0, -1.0), (2.0, 2.0, 1.0))
+    rng = np.random.default_rng(11)
+    f = rng.random((n, n) + nv)
+    # swap (x,y) and (vx,vy): the x sweep of the swapped array is the y sweep of the original
+    ft = np.ascontiguousarray(f.transpose(1, 0, 3, 2, 4))
+    fy = f.copy()
+    assert orc.sweep_y(fy, sp, n, n, 0, 0.5, 0.83, orc.BC_PERIODIC, orc.BC_PERIODIC) == 0
+    orc.sweep_x(ft, sp, n, n, 0, 0.5, 0.83)
+    assert np.array_equal(fy, ft.transpose(1, 0, 3, 2, 4))
+
+
+def test_reflect_wall_equals_periodic_image_domain(orc):
+    """R19 by the method of images: a REFLECT box of ny rows evolves like the upper half of a periodic box of
+    2 ny rows whose lower half holds the mirror image f(-y, vx, -vy, vz)."""
+    nx, ny, nv = 3, 6, (2, 6, 2)
+    sp = _species(orc, nv, (-1.0, -3.0, -1.0), (1.0, 3.0, 1.0))
+    rng = np.random.default_rng(12)
+    f = rng.random((ny, nx) + nv)
+    img = f[::-1, :, :, ::-1, :]
+    big = np.ascontiguousarray(np.concatenate([img, f], axis=0))
+    for dts in (0.11, 0.4, 0.77):          # shifts up to 0.77*2.5/0.5 = 3.85 cells
+        fr, bg = f.copy(), big.copy()
+        assert orc.sweep_y(fr, sp, nx, ny, 0, 0.5, dts, orc.BC_REFLECT, orc.BC_REFLECT) == 0
+        assert orc.sweep_y(bg, sp, nx, 2 * ny, 0, 0.5, dts, orc.BC_PERIODIC, orc.BC_PERIODIC) == 0
+        assert np.abs(fr - bg[ny:]).max() <= 2e-15
+        assert abs(fr.sum() - f.sum()) <= 1e-13 * f.sum()
+
+
+def test_fluid_ghost_rows_are_dirichlet_data(orc):
+    """R16: ghost rows are read, never written; with ghost rows holding the periodic wrap the interior result
+    equals the periodic sweep; R9: a shift that needs rows beyond the ghost rows reports ERR_SHIFT."""
+    nx, ny, g, nv = 3, 8, 3, (2, 4, 2)
+    sp = _species(orc, nv, (-1.0, -2.0, -1.0), (1.0, 2.0, 1.0))
+    rng = np.random.default_rng(13)
+    fi = rng.random((ny, nx) + nv)
+    fg = np.ascontiguousarray(np.concatenate([fi[-g:], fi, fi[:g]], axis=0))
+    fp = fi.copy()
+    ghost_before = (fg[:g].copy(), fg[-g:].copy())
+    dts = 0.3                              # |sigma| <= 1.5*0.3/0.5 = 0.9 -> needs 2 rows, g = 3 suffices
+    assert orc.sweep_y(fg, sp, nx, ny, g, 0.5, dts, orc.BC_FLUID, orc.BC_FLUID) == 0
+    assert orc.sweep_y(fp, sp, nx, ny, 0, 0.5, dts, orc.BC_PERIODIC, orc.BC_PERIODIC) == 0
+    assert np.array_equal(fg[g:-g], fp)
+    assert np.array_equal(fg[:g], ghost_before[0]) and np.array_equal(fg[-g:], ghost_before[1])
+    assert orc.sweep_y(fg, sp, nx, ny, g, 0.5, 1.2, orc.BC_FLUID, orc.BC_FLUID) == orc.ERR_SHIFT
+
+
+def test_x_sweep_covers_ghost_rows(orc):
+    nx, ny, g, nv = 5, 2, 1, (2, 2, 2)
+    sp = _species(orc, nv, (-1.0,) * 3, (1.0,) * 3)
+    rng = np.random.default_rng(14)
+    f = rng.random((ny + 2 * g, nx) + nv)
+    f0 = f.copy()
+    orc.sweep_x(f, sp, nx, ny, g, 1.0, 0.7)
+    for r in range(ny + 2 * g):
+        one = f0[r:r + 1].copy()
+        orc.sweep_x(one, sp, nx, 1, 0, 1.0, 0.7)
+        assert np.array_equal(f[r], one[0])
+        assert not np.array_equal(f[r], f0[r])
+
+
+def _strang_run(orc, nsteps, T=0.8):
+    """1D1V (x, vx) smooth problem with a prescribed travelling-wave E_x(x, t); E passed at mid-step (R11)."""
+    nx, nvx = 64, 128
+    nv = (nvx, 1, 1)
+    sp = _species(orc, nv, (-6.0, -0.5, -0.5), (6.0, 0.5, 0.5), q=-1.0, m=1.0, finf=10.0)
+    lx = 2 * np.pi
+    x = (np.arange(nx) + 0.5) * lx / nx
+    v = -6.0 + (np.arange(nvx) + 0.5) * 12.0 / nvx
+    f = ((1 + 0.2 * np.cos(x))[:, None] * np.exp(-v ** 2 / 2)[None, :]).reshape(1, nx, nvx, 1, 1).copy()
+    dt = T / nsteps
+    Z = np.zeros((3, 1, nx))
+    for n in range(nsteps):
+        E = Z.copy()
+        E[0, 0] = 1.5 * np.sin(x - 0.7 * (n + 0.5) * dt)
+        err, _ = orc.step(f, sp, nx, 1, 0, lx, 1.0, dt, E, Z, limiter=0, want_moments=False)
+        assert err == 0
+    return f
+
+
+def test_T16_strang_splitting_is_second_order(orc):
+    ref = _strang_run(orc, 64)
+    e = [np.abs(_strang_run(orc, n) - ref).max() for n in (2, 4, 8)]
+    r1, r2 = e[0] / e[1], e[1] / e[2]
+    assert 3.3 < r1 < 5.0 and 3.3 < r2 < 5.0, (e, r1, r2)
+
+
+def _landau_run(orc, steps):
+    w = inputs.landau_workload(steps=steps)
+    spec = w.species[0]
+    f = inputs.landau_f(w)
+    sp = orc.Species(spec.q, spec.m, spec.nv, spec.vmin, spec.vmax, spec.f_inf)
+    nx, ny = w.nx, w.ny
+    k = 2 * np.pi * np.fft.fftfreq(nx, d=w.dx)
+    Z = np.zeros((3, ny, nx))
+    m0 = f.sum()
+    t, W = [], []
+    for n in range(steps):
+        # time-centred field (R11): x half step -> moments -> Poisson -> v step -> x half step
+        err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, Z, Z, stages=orc.STAGE_X1)
+        assert err == 0
+        ne = orc.moments(f, sp, nx, ny, 0)[0].mean(axis=0)
+        rho_hat = np.fft.fft(1.0 - ne)                     # d_x E = 1 - n_e  (R20, q_e = -1, fixed ion background)
+        Eh = np.zeros(nx, dtype=complex)
+        Eh[1:] = rho_hat[1:] / (1j * k[1:])
+        Ex = np.fft.ifft(Eh).real
+        E = Z.copy()
+        E[0] = Ex[None, :]
+        err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, E, Z, stages=orc.STAGE_V)
+        assert err == 0
+        err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, Z, Z, stages=orc.STAGE_X2)
+        assert err == 0
+        t.append((n + 0.5) * w.dt)
+        W.append(0.5 * np.sum(Ex ** 2) * w.dx)
+    return np.array(t), np.array(W), abs(f.sum() - m0) / m0
+
+
+def _peaks(t, W):
+    """Local maxima of the field energy, refined by a parabola through three points."""
+    tp, wp = [], []
+    for i in range(1, len(W) - 1):
+        if W[i] > W[i - 1] and W[i] >= W[i + 1]:
+            a, b, c = np.log(W[i - 1]), np.log(W[i]), np.log(W[i + 1])
+            d = 0.5 * (a - c) / (a - 2 * b + c)
+            tp.append(t[i] + d * (t[1] - t[0]))
+            wp.append(b - 0.25 * (a - c) * d)
+    return np.array(tp), np.array(wp)
+
+
+@pytest.mark.slow
+def test_T12_landau_damping_rate(orc):
+    """gamma(k=0.5) = -0.1533, omega = 1.4157 (root of the plasma dispersion relation, textbook value named by
+    BASELINE.json).  W ~ exp(2 gamma t) cos^2(omega t): peaks every pi/omega."""
+    t, W, drift = _landau_run(orc, 400)
+    assert drift <= 1e-13
+    tp, wp = _peaks(t, W)
+    sel = (tp > 2.0) & (tp < 18.5)
+    assert sel.sum() >= 7
+    slope = np.polyfit(tp[sel], wp[sel], 1)[0]
+    gamma = slope / 2
+    omega = np.pi / np.mean(np.diff(tp[sel]))
+    assert abs(gamma + 0.1533) <= 0.004, gamma
+    assert abs(omega - 1.4157) <= 0.005, omega
+    # the 100 steps of configs[0] hold two interior peaks: they pin gamma to about +-8 %
+    first = tp < 5.0
+    assert first.sum() == 2
+    g100 = 0.5 * (wp[first][1] - wp[first][0]) / (tp[first][1] - tp[first][0])
+    assert abs(g100 + 0.1533) <= 0.013, g100
