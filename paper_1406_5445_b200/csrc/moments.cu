@@ -1,0 +1,153 @@
+// a9: velocity moments, eqs. (2)-(4) PAPER.md:39-46 as midpoint sums over the velocity block of one
+// spatial cell (R14: the 10 raw moments M0, M1_d, M2_de, each times dvx dvy dvz), plus max_v f as an
+// 11th output (the ghost fill's f_infinity, R15d).  Current density, eq. (11) PAPER.md:74.
+//
+// One CTA per spatial cell.  A thread owns pairs of neighbouring v_z cells and walks i_vx with three
+// running sums per column (sum f, sum vx f, sum vx^2 f), folded with (vy, vz) once per column: about
+// 3.3 fp64 operations per phase-space cell.  Reduction: warp shuffle, then a fixed-order tree over the
+// warps in shared memory -- no atomics, so reruns are bit-identical.
+#include "vlasov_internal.cuh"
+
+namespace vl {
+
+struct MomParams {
+    const double* __restrict__ f;
+    double* __restrict__ out;   // [11][ncell_out]
+    long S;
+    int nv0, nv1, nv2;
+    double vmin[3], dv[3];
+    int cell0, ncell_out;
+};
+
+constexpr int MOM_THREADS = 256;
+
+__global__ void __launch_bounds__(MOM_THREADS) moments_kernel(MomParams P) {
+    const int cell = P.cell0 + blockIdx.x;
+    const double* fb = P.f + (long)cell * P.S;
+    const int plane = P.nv1 * P.nv2;
+    const int nchunk = plane / 2;
+    double M[10];
+#pragma unroll
+    for (int k = 0; k < 10; ++k) M[k] = 0.0;
+    double mx = 0.0;
+    for (int ch = threadIdx.x; ch < nchunk; ch += MOM_THREADS) {
+        const int col = 2 * ch;
+        const int iy = col / P.nv2, iz = col - iy * P.nv2;
+        const double vy = P.vmin[1] + (iy + 0.5) * P.dv[1];
+        const double vza = P.vmin[2] + (iz + 0.5) * P.dv[2];
+        const double vzb = P.vmin[2] + (iz + 1.5) * P.dv[2];
+        double a0 = 0, a1 = 0, a2 = 0, b0 = 0, b1 = 0, b2 = 0;
+        const double2* p = reinterpret_cast<const double2*>(fb + col);
+        const long pstride = plane / 2;
+#pragma unroll 4
+        for (int k = 0; k < P.nv0; ++k) {
+            const double vx = P.vmin[0] + (k + 0.5) * P.dv[0];
+            const double2 v = __ldcs(p + (long)k * pstride);
+            const double wa = vx * v.x, wb = vx * v.y;
+            a0 += v.x; a1 += wa; a2 += vx * wa;
+            b0 += v.y; b1 += wb; b2 += vx * wb;
+            mx = fmax(mx, fmax(v.x, v.y));
+        }
+        const double s0 = a0 + b0, s1 = a1 + b1, s2 = a2 + b2;
+        const double z0 = vza * a0 + vzb * b0;          // sum vz f
+        const double z1 = vza * a1 + vzb * b1;          // sum vx vz f
+        M[0] += s0;
+        M[1] += s1;
+        M[2] += vy * s0;
+        M[3] += z0;
+        M[4] += s2;
+        M[5] += vy * vy * s0;
+        M[6] += vza * vza * a0 + vzb * vzb * b0;
+        M[7] += vy * s1;
+        M[8] += z1;
+        M[9] += vy * z0;
+    }
+    // warp tree
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) M[k] += __shfl_down_sync(0xffffffffu, M[k], o);
+        mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    }
+    __shared__ double red[MOM_THREADS / 32][11];
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) red[w][k] = M[k];
+        red[w][10] = mx;
+    }
+    __syncthreads();
+    if (threadIdx.x < 11) {
+        const int k = threadIdx.x;
+        double r = red[0][k];
+        for (int ww = 1; ww < MOM_THREADS / 32; ++ww) r = (k < 10) ? r + red[ww][k] : fmax(r, red[ww][k]);
+        if (k < 10) r *= P.dv[0] * P.dv[1] * P.dv[2];
+        P.out[(long)k * P.ncell_out + blockIdx.x] = r;
+    }
+}
+
+int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out, int row0, int nrows) {
+    if (nrows <= 0) return VLASOV_OK;
+    MomParams P;
+    P.f = f; P.out = out; P.S = s.nvtot;
+    P.nv0 = s.nv[0]; P.nv1 = s.nv[1]; P.nv2 = s.nv[2];
+    for (int d = 0; d < 3; ++d) { P.vmin[d] = s.vmin[d]; P.dv[d] = s.dv[d]; }
+    P.cell0 = row0 * c->G.nx;
+    P.ncell_out = nrows * c->G.nx;
+    {
+        Launch L(c, K_MOMENTS);
+        moments_kernel<<<P.ncell_out, MOM_THREADS, 0, c->stream>>>(P);
+    }
+    return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
+}
+
+// ------------------------------------------------------------------------------------------------
+// eq. (11): j = sum_s q_s M1^(s); Yee: interpolated to the E positions of R17
+// ------------------------------------------------------------------------------------------------
+struct CurParams {
+    const double* __restrict__ mom;   // [ns][11][ncell]
+    double* __restrict__ J;
+    double q[MAX_SPECIES];
+    int ns, nx, nyg, fields_yee, wall;
+};
+
+__device__ __forceinline__ double jc_at(const CurParams& P, int d, int j, int i) {
+    const long PL = (long)P.nx * P.nyg;
+    double r = 0.0;
+    for (int s = 0; s < P.ns; ++s) r += P.q[s] * P.mom[((long)s * 11 + 1 + d) * PL + (long)j * P.nx + i];
+    return r;
+}
+
+__global__ void current_kernel(CurParams P) {
+    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ncell = P.nx * P.nyg;
+    if (cell >= ncell) return;
+    const int j = cell / P.nx, i = cell % P.nx;
+    const long PL = ncell;
+    if (!P.fields_yee) {
+        for (int d = 0; d < 3; ++d) P.J[d * PL + cell] = jc_at(P, d, j, i);
+        return;
+    }
+    const int im = (i + P.nx - 1) % P.nx;
+    int jm = j - 1;
+    bool onwall = false;
+    if (jm < 0) { jm = P.nyg - 1; onwall = P.wall != 0; }
+    P.J[0 * PL + cell] = onwall ? 0.0 : 0.5 * (jc_at(P, 0, jm, i) + jc_at(P, 0, j, i));
+    P.J[1 * PL + cell] = 0.5 * (jc_at(P, 1, j, im) + jc_at(P, 1, j, i));
+    P.J[2 * PL + cell] = onwall ? 0.0 : 0.25 * (jc_at(P, 2, jm, im) + jc_at(P, 2, jm, i) + jc_at(P, 2, j, im) + jc_at(P, 2, j, i));
+}
+
+int launch_current(vlasov_ctx* c, double* J) {
+    CurParams P;
+    P.mom = c->mom; P.J = J;
+    P.ns = c->ns; P.nx = c->G.nx; P.nyg = c->G.nyg; P.fields_yee = c->G.fields_yee; P.wall = c->G.wall;
+    for (int s = 0; s < c->ns; ++s) P.q[s] = c->sp[s].q;
+    const int ncell = P.nx * P.nyg;
+    {
+        Launch L(c, K_CURRENT);
+        current_kernel<<<(ncell + 127) / 128, 128, 0, c->stream>>>(P);
+    }
+    return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
+}
+
+}  // namespace vl

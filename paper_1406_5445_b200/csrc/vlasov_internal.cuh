@@ -1,0 +1,140 @@
+// Internal declarations of libvlasov_b200 (CUDA path).  Shares nothing with oracle/.
+// Citations: PAPER.md:<line> + equation; readings R* are in DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/vlasov.h"
+
+namespace vl {
+
+constexpr int MAX_SPECIES = 8;
+// per-spatial-cell sweep table, 16 doubles per cell:
+//   [4*d + 0..3], d = 0,1,2: sigma(k, k1, k2) = c0 + c1*k + c2*k1 + c3*k2 for face k (between cells
+//   k-1 and k) of the line with transverse cell indices (k1, k2) -- d=0: (ivy, ivz); d=1: (ivx, ivz);
+//   d=2: (ivx, ivy).  [12 + d]: f_infinity of sweep d.  [15]: multiplicative scale applied to the
+//   source block before the first sweep (ghost fill), 1 otherwise.  [16]: spatial cell the first sweep
+//   READS (ghost fill: the edge cell, R15a; otherwise the cell itself), stored as a double.
+constexpr int TAB = 20;
+
+struct Species {
+    double q, m;
+    int nv[3];
+    double vmin[3], dv[3];
+    double f_inf;
+    long nvtot;        // nv[0]*nv[1]*nv[2]
+    double* f;         // caller's buffer
+    const double* fluid[2];   // fluid5 of y_lo / y_hi (device), or null
+};
+
+struct Geom {
+    int nx, ny, g, nyg;
+    double dx, dy;
+    int bc_lo, bc_hi;
+    int limiter, fields_yee, wall;
+};
+
+}  // namespace vl
+
+struct vlasov_ctx {
+    vl::Geom G;
+    int order;
+    double c, mu0;
+    int ns;
+    vl::Species sp[vl::MAX_SPECIES];
+    cudaStream_t stream;
+    // scratch carve-up (device)
+    double* pong;        // ping-pong copy of one species' f
+    double* table;       // [nyg*nx][TAB] sweep table (rebuilt per species and stage)
+    double* mom;         // [ns][11][nyg*nx] kept moments (+ max f as the 11th)
+    double* gmom;        // [11][nx] moments of one edge row (ghost fill)
+    double* fields_stage;// [6][nyg*nx] device staging of E,B for vlasov_step_host
+    int* errflag;        // device int: first asynchronous error
+    int mom_valid;
+    int64_t launches;
+    int* h_err;          // pinned host mirror of errflag
+    double* Jbuf;        // [3][nyg*nx] current density of vlasov_cycle
+    double* Bavg;        // [3][nyg*nx] B at the E time level of vlasov_cycle
+    // optional per-kernel timing (vlasov_timing_*): event pairs around every launch
+    int timing;
+    int nrec;
+    static constexpr int MAX_REC = 8192;
+    cudaEvent_t* ev0;    // [MAX_REC]
+    cudaEvent_t* ev1;
+    int* rec_kind;
+};
+
+namespace vl {
+
+enum Kind { K_SWEEP_X = 0, K_SWEEP_Y, K_TABLE, K_VSWEEP_X, K_VSWEEP_YZ, K_MOMENTS, K_GHOST_TABLE, K_CURRENT,
+            K_MAXWELL, K_COUNT };
+
+// Counts a launch and, when timing is on, brackets it with an event pair on the context's stream.
+struct Launch {
+    vlasov_ctx* c; int slot;
+    Launch(vlasov_ctx* ctx, int kind) : c(ctx), slot(-1) {
+        c->launches++;
+        if (c->timing && c->nrec < vlasov_ctx::MAX_REC) {
+            slot = c->nrec++;
+            c->rec_kind[slot] = kind;
+            cudaEventRecord(c->ev0[slot], c->stream);
+        }
+    }
+    ~Launch() { if (slot >= 0) cudaEventRecord(c->ev1[slot], c->stream); }
+};
+
+#define VL_CUDA_OK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return VLASOV_ECUDA; } while (0)
+
+// ---- launchers (each returns VLASOV_OK / VLASOV_ECUDA and bumps ctx->launches) -----------------
+// spatial half sweeps, out of place src -> dst (a1, a2, a7, a8 of DESIGN.md)
+int launch_sweep_x(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);
+int launch_sweep_y(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);
+// Lorentz table (a3) and velocity sweeps (a4-a6), in place on f, rows [row0, row0+nrows)
+int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const double* B, double dt);
+int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows);
+// moments (a9): out[11][nyg*nx] (10 moments + max f) of rows [row0,row0+nrows) of f
+int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out, int row0, int nrows);
+// ghost fill (a0) of one side
+int launch_ghost_fill(vlasov_ctx* c, const Species& s, double* f, int side);
+int launch_current(vlasov_ctx* c, double* J);
+int launch_maxwell(vlasov_ctx* c, double dt, int nsub, double* E, double* B, const double* J, double* Bavg);
+
+// ---- device helpers shared by all sweep kernels ------------------------------------------------
+// Limited slopes of cell j, eqs. (43), (44) PAPER.md:273-276 with R6, written division-free:
+//   eps+ (f_{j+1}-f_j) = clamp(d+, -max(0,Bv), max(0,A)),  eps- (f_j-f_{j-1}) = clamp(d-, -max(0,A), max(0,Bv)),
+//   A = 2 f_j, Bv = 2 (f_inf - f_j).  Algebraically identical to the quotient form.
+__device__ __forceinline__ void limited_slopes(double fm, double f0, double fp, double finf, int limiter,
+                                               double& sp, double& sm) {
+    double dp = fp - f0, dm = f0 - fm;
+    if (limiter) {
+        double A = f0 + f0;
+        double Bv = 2.0 * (finf - f0);
+        double hiA = fmax(A, 0.0), hiB = fmax(Bv, 0.0);
+        sp = fmin(fmax(dp, -hiB), hiA);
+        sm = fmin(fmax(dm, -hiA), hiB);
+    } else {
+        sp = dp; sm = dm;
+    }
+}
+
+// Partial flux of the foot cell: b * [ f_j + (1-b)(2-b)/6 * eps+ d+ + (1-b)(1+b)/6 * eps- d- ],
+// eq. (46) PAPER.md:288 (b = alpha in [0,1]); eq. (47) is the same expression on the mirrored line.
+__device__ __forceinline__ double partial_flux(double fm, double f0, double fp, double b, double finf, int limiter) {
+    double sp, sm;
+    limited_slopes(fm, f0, fp, finf, limiter, sp, sm);
+    double omb = 1.0 - b;
+    double t = omb * (1.0 / 6.0);
+    double c1 = t * (2.0 - b);
+    double c2 = t * (1.0 + b);
+    return b * (f0 + c1 * sp + c2 * sm);
+}
+
+// n = floor(s) for s >= 0 up to the exact-integer case, where n = s - 1, b = 1 is returned instead:
+// the flux is identical there (R8).  Magic-number rounding, no conversion-pipe instruction.
+__device__ __forceinline__ void split_shift(double s, int& n, double& b) {
+    const double M = 6755399441055744.0;   // 1.5 * 2^52
+    double r = (s - 0.5) + M;
+    n = __double2loint(r);
+    b = s - (r - M);
+}
+
+}  // namespace vl

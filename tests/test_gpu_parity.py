@@ -1,0 +1,339 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the same
+seeded inputs.  Tolerances are north_star's: relative L2 <= 1e-12 after one step, <= 1e-10 after 50
+steps, relative mass drift <= 1e-13; moments <= 1e-12."""
+import numpy as np
+import pytest
+
+from paper_1406_5445_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = 1e-12
+TOL50 = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1406_5445_b200 import binding
+    binding.lib()           # fails loudly when the library is missing
+    return binding
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    d = np.linalg.norm(a - b)
+    n = np.linalg.norm(b)
+    return d / n if n > 0 else d
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def osp(orc, s):
+    return orc.Species(s.q, s.m, s.nv, s.vmin, s.vmax, s.f_inf)
+
+
+def random_workload(rng, nx, ny, nv, g=0, bc=inputs.BC_PERIODIC, nspecies=1, fields_yee=0, vmax=(4.0, 3.0, 2.0)):
+    sp = []
+    for s in range(nspecies):
+        q = -1.0 if s == 0 else 1.0
+        m = 1.0 if s == 0 else 4.0
+        sp.append(inputs.SpeciesSpec(f"s{s}", q=q, m=m, nv=tuple(nv), vmin=tuple(-x for x in vmax), vmax=tuple(vmax), f_inf=1.0))
+    w = inputs.Workload("random", nx=nx, ny=ny, nghost_y=g, lx=1.7, ly=0.9, x0=0.0, y0=0.0, bc_y_lo=bc, bc_y_hi=bc,
+                        dt=0.05, steps=1, species=sp, c=3.0, mu0=1.0, nsub=1, fields_yee=fields_yee, seed=3)
+    return w
+
+
+def smooth_random_f(rng, w, s):
+    """Positive, bounded by f_inf = 1, rough enough to exercise the limiters."""
+    sp = w.species[s]
+    shape = (w.ny_g, w.nx) + sp.nv
+    c = [sp.centres(d) for d in range(3)]
+    M = np.exp(-0.5 * ((c[0][:, None, None] / 1.3) ** 2 + (c[1][None, :, None] / 1.1) ** 2 + (c[2][None, None, :] / 0.8) ** 2))
+    f = 0.9 * M[None, None] * (0.3 + 0.7 * rng.random(shape))
+    f[rng.random(shape) < 0.05] = 0.0
+    f[rng.random(shape) < 0.02] = 1.0
+    return np.ascontiguousarray(f)
+
+
+def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None):
+    """One vlasov_step on both sides.  Returns (f_gpu list, f_orc list, mom_gpu list, mom_orc list, code)."""
+    import torch
+    fg = [dev(f) for f in f0]
+    ctx = gpu.context_for(w, fg, order=order, limiter=limiter)
+    keep = []
+    if fluid is not None:
+        for s in range(len(w.species)):
+            for side in (0, 1):
+                t = dev(fluid[s][side])
+                keep.append(t)
+                ctx.vlasov_set_boundary(s, side, inputs.BC_FLUID, t)
+    Ed, Bd = dev(E), dev(B)
+    ctx.vlasov_step(dt, Ed, Bd, stages)
+    code = ctx.check_code()
+    momg = []
+    for s in range(len(w.species)):
+        m = torch.empty((10, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+        ctx.vlasov_moments(s, m)
+        momg.append(m.cpu().numpy())
+    fo, momo = [], []
+    for s, spec in enumerate(w.species):
+        f = f0[s].copy()
+        fl = (None, None) if fluid is None else fluid[s]
+        err, _ = orc.step(f, osp(orc, spec), w.nx, w.ny, w.nghost_y, w.lx, w.ly, dt, E, B, fields_yee=w.fields_yee,
+                          limiter=limiter, bc_lo=w.bc_y_lo, bc_hi=w.bc_y_hi, fluid_lo=fl[0], fluid_hi=fl[1], order=order,
+                          stages=stages, want_moments=False)
+        fo.append(f)
+        momo.append(orc.moments(f, osp(orc, spec), w.nx, w.ny, w.nghost_y))
+    out = [t.cpu().numpy() for t in fg]
+    ctx.close()
+    return out, fo, momg, momo, code
+
+
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_REFLECT])
+@pytest.mark.parametrize("stages", [1, 4])
+def test_spatial_half_steps(gpu, orc, bc, stages):
+    """a1+a2 / a7+a8 on ragged sizes: shifts of both signs, several cells (|sigma| up to ~3.5), wrap-around."""
+    rng = np.random.default_rng(1)
+    w = random_workload(rng, nx=13, ny=9, nv=(6, 8, 10), bc=bc)
+    f0 = [smooth_random_f(rng, w, 0)]
+    Z = np.zeros((3, w.ny_g, w.nx))
+    dt = 0.23         # sigma_x = vx * dt/2 / (1.7/13) up to 3.2 cells; sigma_y up to 3.0 cells
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, Z, Z, dt, stages)
+    assert code == 0
+    assert rel_l2(fg[0], fo[0]) <= TOL1
+    assert np.abs(fg[0] - fo[0]).max() <= 1e-13
+    assert rel_l2(mg[0], mo[0]) <= TOL1
+
+
+@pytest.mark.parametrize("fields_yee", [0, 1])
+def test_velocity_step_multicell_shifts(gpu, orc, fields_yee):
+    """a3-a6: strong fields give sign-changing shifts of several cells; Yee gather vs cell-centred."""
+    rng = np.random.default_rng(2)
+    w = random_workload(rng, nx=5, ny=4, nv=(12, 10, 14), bc=inputs.BC_REFLECT, fields_yee=fields_yee)
+    f0 = [smooth_random_f(rng, w, 0)]
+    E = 6.0 * rng.standard_normal((3, w.ny_g, w.nx))
+    B = 8.0 * rng.standard_normal((3, w.ny_g, w.nx))
+    B *= 0.9 / (np.abs(B).max() * 0.5 * 0.1)        # |t| = |q/m dt/2 B| up to 0.9 per component? keep D1, D2 > 0
+    B *= 0.5
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, 0.1, 2)
+    assert code == 0
+    assert rel_l2(fg[0], fo[0]) <= TOL1
+    assert rel_l2(mg[0], mo[0]) <= TOL1
+    # the sweep really moved things by more than a cell somewhere
+    assert np.abs(fg[0] - f0[0]).max() > 0.1
+
+
+@pytest.mark.parametrize("order", [0, 1])
+@pytest.mark.parametrize("limiter", [1, 0])
+def test_full_step_two_species(gpu, orc, order, limiter):
+    rng = np.random.default_rng(3)
+    w = random_workload(rng, nx=9, ny=6, nv=(8, 8, 8), bc=inputs.BC_REFLECT, nspecies=2, fields_yee=1)
+    f0 = [smooth_random_f(rng, w, s) for s in range(2)]
+    E = rng.standard_normal((3, w.ny_g, w.nx))
+    B = 2.0 * rng.standard_normal((3, w.ny_g, w.nx))
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, 0.07, 31, order=order, limiter=limiter)
+    assert code == 0
+    for s in range(2):
+        assert rel_l2(fg[s], fo[s]) <= TOL1
+        assert rel_l2(mg[s], mo[s]) <= TOL1
+        m0 = f0[s].sum()
+        assert abs(fg[s].sum() - m0) / m0 <= 1e-13
+
+
+def test_gem_cut_one_step(gpu, orc):
+    """A 16x8 spatial cut of config 2 (GEM Harris sheet, 16^3 velocity cells, both species, Yee fields, REFLECT)."""
+    w = inputs.gem_workload(nx=16, ny=8, nv=16, steps=1)
+    f0 = []
+    for s in range(2):
+        f0.append(inputs.gem_f(w, s))
+        w.species[s].f_inf = inputs.gem_f_inf(w, s)
+    E, B = inputs.gem_fields(w)
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, w.dt, 31)
+    assert code == 0
+    for s in range(2):
+        assert rel_l2(fg[s], fo[s]) <= TOL1, s
+        assert rel_l2(mg[s], mo[s]) <= TOL1, s
+        m0 = f0[s].sum()
+        assert abs(fg[s].sum() - m0) / m0 <= 1e-13
+
+
+def test_ghost_fill_band(gpu, orc):
+    """a0 on a cut of config 4: FLUID sides, 3 ghost rows, seeded fluid state; ghost rows and interior."""
+    w = inputs.band_workload(nx=16, ny_band=8, ny_domain=128, nv=16, g=3)
+    f0 = []
+    for s in range(2):
+        f0.append(inputs.gem_f(w, s))
+        w.species[s].f_inf = inputs.gem_f_inf(w, s)
+    E, B = inputs.gem_fields(w)
+    fluid = [[inputs.band_fluid_state(w, s, side, 0) for side in (0, 1)] for s in range(2)]
+    # ghost fill alone
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, w.dt, 8, fluid=fluid)
+    assert code == 0
+    g = w.nghost_y
+    for s in range(2):
+        for rows in (slice(0, g), slice(g + w.ny, w.ny_g)):
+            assert rel_l2(fg[s][rows], fo[s][rows]) <= TOL1
+            assert np.abs(fg[s][rows] - f0[s][rows]).max() > 0          # it did something
+        assert np.array_equal(fg[s][g:g + w.ny], f0[s][g:g + w.ny])     # interior untouched
+    # whole step with ghost rows as Dirichlet data
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, w.dt, 31, fluid=fluid)
+    assert code == 0
+    for s in range(2):
+        assert rel_l2(fg[s], fo[s]) <= TOL1
+        assert rel_l2(mg[s], mo[s]) <= TOL1
+
+
+def test_free_streaming_integer_shifts_exact_on_gpu(gpu):
+    """T10 on the GPU: integer CFL shifts translate f exactly (no oracle involved)."""
+    import torch
+    nx, ny, nv = 12, 10, (4, 4, 2)
+    sp = inputs.SpeciesSpec("e", -1.0, 1.0, nv, (-4.0, -1.0, -1.0), (4.0, 1.0, 1.0), f_inf=1.0)
+    w = inputs.Workload("fs", nx=nx, ny=ny, nghost_y=0, lx=12.0, ly=2.5, x0=0, y0=0, bc_y_lo=0, bc_y_hi=0, dt=2.0,
+                        steps=1, species=[sp], fields_yee=0)
+    rng = np.random.default_rng(10)
+    f0 = rng.random((ny, nx) + nv)
+    fg = [dev(f0)]
+    ctx = gpu.context_for(w, fg)
+    Z = torch.zeros((3, ny, nx), dtype=torch.float64, device="cuda")
+    ctx.vlasov_step(2.0, Z, Z, 31)
+    ctx.vlasov_check()
+    f = fg[0].cpu().numpy()
+    vx = sp.centres(0)
+    vy = sp.centres(1)
+    for a in range(nv[0]):
+        for b in range(nv[1]):
+            sx = int(round(vx[a] * 2.0 / 1.0))
+            sy = int(round(vy[b] * 2.0 / 0.25))
+            want = np.roll(f0[:, :, a, b, :], (sy, sx), axis=(0, 1))
+            assert np.abs(f[:, :, a, b, :] - want).max() <= 1e-14
+
+
+def test_uniform_maxwellian_invariant_bitwise_on_gpu(gpu):
+    """T11 on the GPU."""
+    import torch
+    nx, ny, nv = 6, 5, (8, 8, 8)
+    sp = inputs.SpeciesSpec("e", -1.0, 1.0, nv, (-6.0,) * 3, (6.0,) * 3, f_inf=1.0)
+    c = sp.centres(0)
+    g = np.exp(-c ** 2 / 2) / np.sqrt(2 * np.pi)
+    M = g[:, None, None] * g[None, :, None] * g[None, None, :]
+    f0 = np.ascontiguousarray(np.broadcast_to(M, (ny, nx) + nv))
+    sp.f_inf = float(f0.max())
+    for bc in (0, 1):
+        w = inputs.Workload("um", nx=nx, ny=ny, nghost_y=0, lx=3.0, ly=2.0, x0=0, y0=0, bc_y_lo=bc, bc_y_hi=bc, dt=0.37,
+                            steps=1, species=[sp], fields_yee=0)
+        fg = [dev(f0)]
+        ctx = gpu.context_for(w, fg)
+        Z = torch.zeros((3, ny, nx), dtype=torch.float64, device="cuda")
+        ctx.vlasov_step(0.37, Z, Z, 31)
+        ctx.vlasov_check()
+        assert np.array_equal(fg[0].cpu().numpy(), f0)
+
+
+def _poisson_E(ne_row, nx, dx):
+    k = 2 * np.pi * np.fft.fftfreq(nx, d=dx)
+    rho_hat = np.fft.fft(1.0 - ne_row)
+    Eh = np.zeros(nx, dtype=complex)
+    Eh[1:] = rho_hat[1:] / (1j * k[1:])
+    return np.fft.ifft(Eh).real
+
+
+def test_landau_config1_50_steps(gpu, orc):
+    """configs[0]: 1 step <= 1e-12, 50 steps <= 1e-10, mass drift <= 1e-13; time-centred Poisson on the host (R11)
+    computed by the same harness code from each side's own moments."""
+    import torch
+    w = inputs.landau_workload(steps=50)
+    spec = w.species[0]
+    f0 = inputs.landau_f(w)
+    sp = osp(orc, spec)
+    nx, ny = w.nx, w.ny
+    fo = f0.copy()
+    fg = [dev(f0)]
+    ctx = gpu.context_for(w, fg)
+    mom = torch.empty((10, ny, nx), dtype=torch.float64, device="cuda")
+    Z = np.zeros((3, ny, nx))
+    Zd = dev(Z)
+    m0 = f0.sum()
+    for n in range(50):
+        orc.step(fo, sp, nx, ny, 0, w.lx, w.ly, w.dt, Z, Z, stages=orc.STAGE_X1, want_moments=False)
+        Eo = Z.copy()
+        Eo[0] = _poisson_E(orc.moments(fo, sp, nx, ny, 0)[0].mean(axis=0), nx, w.dx)[None, :]
+        orc.step(fo, sp, nx, ny, 0, w.lx, w.ly, w.dt, Eo, Z, stages=orc.STAGE_V, want_moments=False)
+        orc.step(fo, sp, nx, ny, 0, w.lx, w.ly, w.dt, Z, Z, stages=orc.STAGE_X2, want_moments=False)
+
+        ctx.vlasov_step(w.dt, Zd, Zd, gpu.STAGE_X1)
+        ctx.vlasov_moments(0, mom)
+        Eg = Z.copy()
+        Eg[0] = _poisson_E(mom[0].cpu().numpy().mean(axis=0), nx, w.dx)[None, :]
+        ctx.vlasov_step(w.dt, dev(Eg), Zd, gpu.STAGE_V)
+        ctx.vlasov_step(w.dt, Zd, Zd, gpu.STAGE_X2)
+        if n == 0:
+            ctx.vlasov_check()
+            assert rel_l2(fg[0].cpu().numpy(), fo) <= TOL1
+    ctx.vlasov_check()
+    out = fg[0].cpu().numpy()
+    assert rel_l2(out, fo) <= TOL50
+    assert abs(out.sum() - m0) / m0 <= 1e-13
+
+
+def test_maxwell_and_current(gpu, orc):
+    import torch
+    rng = np.random.default_rng(5)
+    for bc, yee in ((inputs.BC_PERIODIC, 1), (inputs.BC_REFLECT, 1), (inputs.BC_REFLECT, 0)):
+        w = random_workload(rng, nx=11, ny=7, nv=(4, 4, 4), bc=bc, nspecies=2, fields_yee=yee)
+        f0 = [smooth_random_f(rng, w, s) for s in range(2)]
+        fg = [dev(f) for f in f0]
+        ctx = gpu.context_for(w, fg)
+        J = torch.empty((3, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+        ctx.vlasov_current(J)
+        moms = [orc.moments(f0[s], osp(orc, w.species[s]), w.nx, w.ny, 0) for s in range(2)]
+        wall = 0 if bc == inputs.BC_PERIODIC else 1
+        Jo = orc.current(moms, [s.q for s in w.species], fields_yee=yee, wall=wall)
+        assert rel_l2(J.cpu().numpy(), Jo) <= TOL1
+        E = rng.standard_normal((3, w.ny_g, w.nx))
+        B = rng.standard_normal((3, w.ny_g, w.nx))
+        if wall:
+            E[0, 0] = 0; E[2, 0] = 0; B[1, 0] = 0
+        Eo, Bo = E.copy(), B.copy()
+        Bavg_o = orc.maxwell(Eo, Bo, Jo, w.dx, w.dy, w.c, w.mu0, 0.01, 4, wall, want_bavg=True)
+        Ed, Bd, Bavg = dev(E), dev(B), torch.empty((3, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+        ctx.vlasov_maxwell(0.01, 4, Ed, Bd, dev(Jo), Bavg)
+        ctx.vlasov_check()
+        assert rel_l2(Ed.cpu().numpy(), Eo) <= 1e-14
+        assert rel_l2(Bd.cpu().numpy(), Bo) <= 1e-14
+        assert rel_l2(Bavg.cpu().numpy(), Bavg_o) <= 1e-14
+        ctx.close()
+
+
+def test_error_paths(gpu, orc):
+    import torch
+    rng = np.random.default_rng(6)
+    # ESHIFT: FLUID side with one ghost row and a shift that needs more (R9)
+    w = random_workload(rng, nx=4, ny=6, nv=(4, 4, 4), g=1, bc=inputs.BC_FLUID)
+    f0 = [smooth_random_f(rng, w, 0)]
+    fg = [dev(f0[0])]
+    ctx = gpu.context_for(w, fg)
+    Z = torch.zeros((3, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+    ctx.vlasov_step(0.05, Z, Z, gpu.STAGE_X1)
+    assert ctx.check_code() == gpu.ESHIFT
+    assert ctx.check_code() == 0          # cleared
+    # EDOMAIN: |t| > 1 makes a Boris denominator non-positive (R13)
+    Bbig = torch.zeros((3, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+    Bbig[0] = 100.0
+    ctx.vlasov_step(0.05, Z, Bbig, gpu.STAGE_V)
+    assert ctx.check_code() == gpu.EDOMAIN
+    ctx.close()
+    # EINVAL / EALIGN at init
+    cfg = gpu.make_config(4, 4, 0, 1, 1.0, 1.0, 0, 0)
+    sp = gpu.make_species(w.species)
+    with pytest.raises(gpu.VlasovError) as e:
+        gpu.Context(cfg, sp, [torch.zeros(4 * 4 * 64 + 2, dtype=torch.float64, device="cuda")[1:-1]])
+    assert e.value.code == gpu.EALIGN
+    cfg2 = gpu.make_config(0, 4, 0, 1, 1.0, 1.0, 0, 0)
+    assert gpu.vlasov_scratch_bytes(cfg2, sp) == 0
