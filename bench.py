@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the Vlasov full-step hot path on B200.
+
+A "step" is one cycle of section 4.3 without the fluid solve, for all species:
+currents (eq. 11) -> Maxwell half step -> one complete Vlasov step (x/2, y/2, vx, vy, vz, y/2, x/2, eq. 22)
+with its moment reductions -> currents -> Maxwell half step; plus the ghost fill where a y side is FLUID.
+metric = interior phase-space cell-updates/s (all species).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload gem128|gem64|band|nv16|nv24|nv32|nv48]
+    python bench.py --impl reference ...     # the oracle, as it stands, on the host cores (rank 0 only)
+
+Prints ONE JSON line (rank 0).  N > 1 = N independent replicas (the build is single-GPU by north_star,
+DESIGN.md "Multi-GPU": replicas only, no collective on the data path); launched by torchrun.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+from paper_1406_5445_b200 import inputs
+
+METRIC = "vlasov_phase_space_cell_updates_per_s"
+UNIT = "cell-updates/s"
+
+# Algorithmic HBM bytes per phase-space cell and launch of each f-sized kernel:
+# a sweep reads and writes every cell once (8 + 8 B); the moments pass reads it once.
+BYTES_PER_CELL = {"sweep_x": 16.0, "sweep_y": 16.0, "sweep_xy": 16.0, "vsweep_x": 16.0, "vsweep_yz": 16.0,
+                  "vsweep_xyz": 16.0, "moments": 8.0}
+
+
+def make_workload(name):
+    if name == "gem128":
+        return inputs.gem_workload(nx=128, ny=64, nv=32, steps=20, name="gem_128x64x32^3_x2species")
+    if name == "gem64":
+        return inputs.gem_workload(nx=64, ny=32, nv=32, steps=50, name="gem_64x32x32^3_x2species")
+    if name == "band":
+        return inputs.band_workload()
+    if name.startswith("nv"):
+        nv = int(name[2:])
+        return inputs.gem_workload(nx=64, ny=64, nv=nv, steps=10, name=f"gem_64x64x{nv}^3_x2species")
+    raise SystemExit(f"unknown workload {name}")
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks sampled DURING the timed region
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,power.draw")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index):
+        self.lines = []
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.p = None
+
+    def _read(self):
+        for ln in self.p.stdout:
+            self.lines.append((time.time(), ln.strip()))
+
+    def stop(self, t0, t1):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        rows = [ln for (t, ln) in self.lines if t0 <= t <= t1 + 0.12] or [ln for (_, ln) in self.lines[-3:]]
+        for ln in rows:
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[6]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(self.NAMES):
+                if c[2 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm), "power_w_max": max(pw) if pw else None}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference): only oracle/ is executed here
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_workload(w, nx_s=16, ny_s=8):
+    """A bounded sample of workload w: the same species, velocity grids, dt, dx, dy, profiles and noise on
+    an nx_s x ny_s spatial cut around the sheet centre (y rows straddle y = 0)."""
+    nx_s = min(nx_s, w.nx)
+    ny_s = min(ny_s, w.ny)
+    import copy
+    ws = copy.deepcopy(w)
+    ws.nx, ws.ny = nx_s, ny_s
+    ws.lx, ws.ly = w.dx * nx_s, w.dy * ny_s
+    ws.x0, ws.y0 = -ws.lx / 2, -ws.ly / 2
+    ws.ly_domain = getattr(w, "ly_domain", w.ly)
+    ws.name = f"{w.name}:cut{nx_s}x{ny_s}"
+    return ws
+
+
+class OracleRun:
+    """The section-4.3 cycle composed from the oracle's own functions (no CUDA)."""
+
+    def __init__(self, ws):
+        from oracle import oracle as orc
+        self.orc, self.w = orc, ws
+        orc.build()
+        self.sp = []
+        self.f = []
+        for s, spec in enumerate(ws.species):
+            self.f.append(inputs.gem_f(ws, s))
+            spec.f_inf = inputs.gem_f_inf(ws, s)
+            self.sp.append(orc.Species(spec.q, spec.m, spec.nv, spec.vmin, spec.vmax, spec.f_inf))
+        self.E, self.B = inputs.gem_fields(ws)
+        self.wall = 0 if ws.bc_y_lo == inputs.BC_PERIODIC else 1
+        self.fluid = None
+        self.mom = [orc.moments(f, sp, ws.nx, ws.ny, ws.nghost_y) for f, sp in zip(self.f, self.sp)]
+        self.step_index = 0
+
+    def cycle(self):
+        orc, w = self.orc, self.w
+        q = [sp.q for sp in self.sp]
+        J = orc.current(self.mom, q, w.fields_yee, self.wall)
+        Bavg = orc.maxwell(self.E, self.B, J, w.dx, w.dy, w.c, w.mu0, w.dt / 2, w.nsub, self.wall, want_bavg=True)
+        for s, sp in enumerate(self.sp):
+            fl = (None, None)
+            if w.bc_y_lo == inputs.BC_FLUID:
+                fl = (inputs.band_fluid_state(w, s, 0, self.step_index), inputs.band_fluid_state(w, s, 1, self.step_index))
+            err, m = orc.step(self.f[s], sp, w.nx, w.ny, w.nghost_y, w.lx, w.ly, w.dt, self.E, Bavg,
+                              fields_yee=w.fields_yee, bc_lo=w.bc_y_lo, bc_hi=w.bc_y_hi, fluid_lo=fl[0], fluid_hi=fl[1])
+            if err:
+                raise RuntimeError(f"oracle step error {err}")
+            self.mom[s] = m
+        J = orc.current(self.mom, q, w.fields_yee, self.wall)
+        orc.maxwell(self.E, self.B, J, w.dx, w.dy, w.c, w.mu0, w.dt / 2, w.nsub, self.wall)
+        self.step_index += 1
+
+
+def oracle_leg(w, steps, warmup, budget_s=25.0):
+    """Time the oracle on a bounded sample.  Returns (cell-updates/s, ms/step, cores, sample text, steps done)."""
+    ws = oracle_sample_workload(w)
+    run = OracleRun(ws)
+    cores = run.orc.num_threads()
+    for _ in range(warmup):
+        run.cycle()
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(steps):
+        run.cycle()
+        done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    cells = ws.interior_cells
+    sample = (f"{ws.nx}x{ws.ny} spatial cut of {w.name} (same species, {ws.species[0].nv[0]}^3 velocity cells each, dt, dx, dy, "
+              f"profiles, noise), {done} full cycle(s) after {warmup} warm-up, {cells} interior cells/step")
+    return cells * done / dt, 1e3 * dt / done, cores, sample, done
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+def upload_f(w, s, torch, device):
+    """Seeded f of species s, generated row by row on the host and copied to the device."""
+    sp = w.species[s]
+    f = torch.empty((w.ny_g, w.nx) + tuple(sp.nv), dtype=torch.float64, device=device)
+    for r in range(w.ny_g):
+        f[r].copy_(torch.from_numpy(inputs.gem_f(w, s, rows=[r])[0]))
+    sp.f_inf = inputs.gem_f_inf(w, s)
+    return f
+
+
+def gpu_arm(args):
+    import torch
+    from paper_1406_5445_b200 import binding
+    binding.lib()                                  # fails loudly if the CUDA library is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus and world > 1:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+
+    w = make_workload(args.workload)
+    ns = len(w.species)
+    fs = [upload_f(w, s, torch, device) for s in range(ns)]
+    E0, B0 = inputs.gem_fields(w)
+    stream = torch.cuda.current_stream()
+    ctx = binding.context_for(w, fs)
+    Ed, Bd = torch.from_numpy(E0).to(device), torch.from_numpy(B0).to(device)
+    fluid = None
+    if w.bc_y_lo == inputs.BC_FLUID:
+        # seeded 5-moment states, redrawn per step from the step index (config 4); resident before timing
+        nstate = args.warmup + args.steps + 2 * args.steps + 8
+        fluid = [[[torch.from_numpy(inputs.band_fluid_state(w, s, side, k)).to(device) for side in (0, 1)]
+                  for s in range(ns)] for k in range(nstate)]
+    step_no = [0]
+
+    def set_fluid():
+        if fluid is not None:
+            st = fluid[step_no[0] % len(fluid)]
+            for s in range(ns):
+                for side in (0, 1):
+                    ctx.vlasov_set_boundary(s, side, inputs.BC_FLUID, st[s][side])
+        step_no[0] += 1
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident leg: `value` -------------------------------------------------------
+    for _ in range(args.warmup):
+        set_fluid()
+        ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+    ctx.vlasov_check()
+    ctx.vlasov_timing_enable(True)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = ctx.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall0 = time.time()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        set_fluid()
+        ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+    ev1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    ctx.vlasov_check()
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms = ev0.elapsed_time(ev1)
+    per_kind = ctx.vlasov_timing_read()
+    ctx.vlasov_timing_enable(False)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    cells = w.interior_cells
+    value = world * cells * args.steps / (ms * 1e-3)
+
+    # ---- end-to-end leg: HOST buffers through the C ABI (vlasov_cycle_host) -----------------
+    ncell = w.ny_g * w.nx
+    Eh = torch.from_numpy(E0.copy()).pin_memory()
+    Bh = torch.from_numpy(B0.copy()).pin_memory()
+    Mh = torch.empty((ns, 10, w.ny_g, w.nx), dtype=torch.float64).pin_memory()
+    Eh.copy_(Ed.cpu()); Bh.copy_(Bd.cpu())
+    e2e_steps = max(1, min(args.steps, 10))
+    set_fluid()
+    ctx.vlasov_cycle_host(w.dt, w.nsub, Eh, Bh, Mh)
+    barrier()
+    ev0.record(stream)
+    for _ in range(e2e_steps):
+        set_fluid()
+        ctx.vlasov_cycle_host(w.dt, w.nsub, Eh, Bh, Mh)
+    ev1.record(stream)
+    barrier()
+    ms_e = ev0.elapsed_time(ev1)
+    if dist is not None:
+        t = torch.tensor([ms_e], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e = float(t.item())
+    e2e = world * cells * e2e_steps / (ms_e * 1e-3)
+    h2d = 6 * ncell * 8
+    d2h = (6 + 10 * ns) * ncell * 8
+    if not np.isfinite(Mh.numpy()).all():
+        raise SystemExit("bench.py: non-finite moments")
+
+    if rank != 0:
+        ctx.close()
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (CUDA-event pairs around every launch, timed region) ----
+    peak, peak_src = peaks()
+    cells_all = sum(w.ny_g * w.nx * s.ncell_v for s in w.species) / ns      # ghost-inclusive, per species launch
+    kinds = {}
+    tot_ms = sum(v[0] for v in per_kind.values())
+    for k, (kms, cnt) in per_kind.items():
+        if cnt == 0:
+            continue
+        ent = {"ms_per_step": kms / args.steps, "launches_per_step": cnt / args.steps, "share": kms / tot_ms}
+        if k in BYTES_PER_CELL:
+            # vsweep/moments launches that only cover ghost rows or one edge row (ghost fill) are small; the
+            # average below is over launches of this kind, bytes are summed over what each launch covers
+            # (with FLUID sides some launches of a kind cover only ghost rows: no per-launch figure then)
+            bytes_total = BYTES_PER_CELL[k] * cells_all * cnt if fluid is None else None
+            if bytes_total is not None:
+                ent["gbs"] = bytes_total / (kms * 1e-3) / 1e9
+                ent["frac_of_peak"] = ent["gbs"] / peak
+        kinds[k] = ent
+    dom = max((k for k in kinds if "gbs" in kinds[k]), key=lambda k: kinds[k]["share"], default=None)
+    roofline = None
+    if dom is not None:
+        d = kinds[dom]
+        roofline = {"kernel": dom, "bound": "hbm", "achieved": d["gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": d["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": BYTES_PER_CELL[dom] * cells_all,
+                    "avg_launch_ms": d["ms_per_step"] / d["launches_per_step"], "share_of_step": d["share"]}
+        tr = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tr):
+            with open(tr) as fh:
+                tj = json.load(fh)
+            if tj.get("workload") == w.name and dom in tj.get("dram_bytes_per_launch", {}):
+                roofline["traffic"] = tj["dram_bytes_per_launch"][dom]
+                roofline["traffic_source"] = tj.get("source")
+    pass_bytes = sum(BYTES_PER_CELL[k] * v["launches_per_step"] / ns for k, v in kinds.items() if k in BYTES_PER_CELL)
+
+    # ---- the oracle timed beside it (reported baseline only) --------------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        v, _, cores, sample, _ = oracle_leg(make_workload(args.workload), steps=50, warmup=1, budget_s=args.cpu_budget)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise, DESIGN.md 'Input recipe')",
+        "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nghost_y": w.nghost_y,
+                   "nv": list(w.species[0].nv), "species": ns, "dt": w.dt, "maxwell_nsub": w.nsub,
+                   "interior_cells_per_step": cells, "order": "XVX (eq. 22)", "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": f"inputs larger than L2: {sum(f.numel() for f in fs) * 8 / 1e9:.2f} GB of f streamed by every pass (L2 126 MB)"},
+        "clocks": clocks,
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                "ms_per_step": ms_e / e2e_steps,
+                "what": "vlasov_cycle_host: E,B from pinned host memory each step, E,B and all moments back; f resident (PAPER.md:86)"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "step_hbm": {"algorithmic_bytes_per_cell_update": pass_bytes,
+                     "achieved_gbs": pass_bytes * cells_all * ns * args.steps / (ms * 1e-3) / 1e9,
+                     "note": "sum over the step's f-sized passes (ghost-inclusive cells) / step time"},
+        "kernels": kinds,
+        "cpu_baseline": cpu,
+    }
+    out["step_hbm"]["frac_of_peak"] = out["step_hbm"]["achieved_gbs"] / peak
+    print(json.dumps(out))
+    ctx.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def reference_arm(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = make_workload(args.workload)
+    v, ms, cores, sample, done = oracle_leg(w, steps=args.steps, warmup=args.warmup, budget_s=150.0)
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+           "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise)",
+           "config": {"workload": w.name, "sample": sample},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="gem128")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        reference_arm(args)
+    else:
+        gpu_arm(args)
+
+
+if __name__ == "__main__":
+    main()
