@@ -116,178 +116,245 @@ int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const
 }
 
 // ------------------------------------------------------------------------------------------------
-// flux through the upper face of cell k (k = 0..N-2) of a line held in shared memory
-//   A[base + j*st], j = 0..N-1, zero outside (R7).  eq. (46) for sigma >= 0, eq. (47) for sigma < 0.
+// Flux through face k (between cells k-1 and k, 1 <= k <= N-1) of a ZERO-PADDED line in shared memory:
+// L points at cell 0, stride st, and cells -3..-1 and N..N+2 hold zeros (f = 0 outside the velocity box,
+// R7), so the three reads around the foot cell need no bounds checks.  eq. (46) for sigma >= 0, eq. (47)
+// (sum repaired, R5) for sigma < 0: the same expression on the mirrored line.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double face_flux(const double* A, int base, int st, int N, int k, double sigma,
-                                            double finf, int limiter) {
+template <int LIM>
+__device__ __forceinline__ double face_flux_pad(const double* __restrict__ L, int st, int N, int k, double sigma,
+                                                double finf) {
     const bool pos = sigma >= 0.0;
-    double s = fmin(fabs(sigma), (double)(N + 3));
+    const double s = fmin(fabs(sigma), (double)(N + 4));
     int n; double b;
     split_shift(s, n, b);
     const int u = pos ? 1 : -1;
-    const int j = pos ? k - n : k + 1 + n;          // foot cell
-    int m = pos ? k - n + 1 : k + 1;                // whole cells between foot cell and face, ascending
+    int j = pos ? k - 1 - n : k + n;                 // foot cell
+    const int m0 = pos ? j + 1 : k;                  // the n whole cells between foot cell and face
+    const int lo = max(m0, 0), hi = min(m0 + n, N);
     double sum = 0.0;
-    for (int r = 0; r < n; ++r, ++m) sum += (m >= 0 && m < N) ? A[base + m * st] : 0.0;
-    const int jm = j - u, jp = j + u;
-    const double fm = (jm >= 0 && jm < N) ? A[base + jm * st] : 0.0;
-    const double f0 = (j >= 0 && j < N) ? A[base + j * st] : 0.0;
-    const double fp = (jp >= 0 && jp < N) ? A[base + jp * st] : 0.0;
-    const double phi = sum + partial_flux(fm, f0, fp, b, finf, limiter);
+    for (int m = lo; m < hi; ++m) sum += L[m * st];
+    j = min(max(j, -2), N + 1);
+    const double f0 = L[j * st];
+    const double fm = L[(j - u) * st];
+    const double fp = L[(j + u) * st];
+    const double phi = sum + partial_flux(fm, f0, fp, b, finf, LIM);
     return pos ? phi : -phi;
 }
 
-// ------------------------------------------------------------------------------------------------
-// a4: vx sweep.  grid = (tiles of CT contiguous (ivy,ivz) cells, spatial cells).
-// ------------------------------------------------------------------------------------------------
+// One thread remaps cells [a, b) of one line: flux per face, eq. (38) per cell.  sigma of face k is
+// s0 + s1 k.  put(i, value) stores the new cell average.
+template <int LIM, class Put>
+__device__ __forceinline__ void march_cells(const double* __restrict__ L, int st, int N, int a, int b, double s0,
+                                            double s1, double finf, Put put) {
+    double kd = (double)a;
+    double phi_lo = a > 0 ? face_flux_pad<LIM>(L, st, N, a, fma(s1, kd, s0), finf) : 0.0;
+#pragma unroll 2
+    for (int i = a; i < b; ++i) {
+        kd += 1.0;
+        const double phi_hi = i + 1 < N ? face_flux_pad<LIM>(L, st, N, i + 1, fma(s1, kd, s0), finf) : 0.0;
+        put(i, L[i * st] + (phi_lo - phi_hi));       // eq. (38): f + (Phi_{i-1/2} - Phi_{i+1/2})
+        phi_lo = phi_hi;
+    }
+}
+
 struct VParams {
     double* __restrict__ f;
     const double* __restrict__ table;
     long S;
     int nv0, nv1, nv2;
     int cell0;        // first spatial cell (ghost-inclusive linear index) of this launch
-    int limiter;
     int ct;           // columns per tile (vx kernel) / planes per tile (vyz kernel)
     int ntile;        // tiles per spatial cell
+    int ntot;         // tiles of this launch
+    int nseg;         // threads per line
 };
 
-__global__ void __launch_bounds__(256) vsweep_x_kernel(VParams P) {
+constexpr int V_THREADS = 256;
+
+// ------------------------------------------------------------------------------------------------
+// a4: vx sweep.  Tile = all i_vx x CT contiguous (i_vy,i_vz) columns, rows -3..-1 and N..N+2 zero.
+// One thread marches a segment of one column; a warp reads/writes 256 contiguous bytes per step.
+// Persistent: a CTA loops over tiles, the pad rows are zeroed once.
+// ------------------------------------------------------------------------------------------------
+template <int LIM>
+__global__ void __launch_bounds__(V_THREADS) vsweep_x_kernel(VParams P) {
     extern __shared__ double sm[];
-    const int CT = P.ct, N = P.nv0;
+    const int CT = P.ct, N = P.nv0, H = CT >> 1;
     const int plane = P.nv1 * P.nv2;
-    double* A = sm;
-    double* Phi = sm + (long)N * CT;
-    const int cell = P.cell0 + blockIdx.x / P.ntile;
-    const int c0 = (blockIdx.x % P.ntile) * CT;
-    const int ncol = min(CT, plane - c0);
-    double* fb = P.f + (long)cell * P.S + c0;
-    const double* T = P.table + (long)cell * TAB;
-    const double t0 = T[0], t1 = T[1], t2 = T[2], t3 = T[3], finf = T[12], scale = T[15];
-    const double* fsrc = P.f + (long)T[16] * P.S + c0;
-    const int tot = N * CT;
-    for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-        int k = e / CT, c = e - k * CT;
-        A[e] = c < ncol ? fsrc[(long)k * plane + c] * scale : 0.0;
-    }
-    __syncthreads();
-    for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-        int k = e / CT, c = e - k * CT;
-        double phi = 0.0;
-        if (k < N - 1 && c < ncol) {
-            int col = c0 + c;
-            int k1 = col / P.nv2, k2 = col - k1 * P.nv2;
-            double sigma = t0 + t1 * (k + 1) + t2 * k1 + t3 * k2;
-            phi = face_flux(A, c, CT, N, k, sigma, finf, P.limiter);
+    double* A = sm + 3 * CT;
+    for (int e = threadIdx.x; e < 3 * CT; e += V_THREADS) { sm[e] = 0.0; A[N * CT + e] = 0.0; }
+    const int seglen = (N + P.nseg - 1) / P.nseg;
+    for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x) {
+        const int cell = P.cell0 + tile / P.ntile;
+        const int c0 = (tile % P.ntile) * CT;
+        const int ncol = min(CT, plane - c0);
+        const double* T = P.table + (long)cell * TAB;
+        const double t0 = T[0], t1 = T[1], t2 = T[2], t3 = T[3], finf = T[12], scale = T[15];
+        const double* fsrc = P.f + (long)T[16] * P.S + c0;
+        double* fb = P.f + (long)cell * P.S + c0;
+        for (int e = threadIdx.x; e < N * H; e += V_THREADS) {
+            const int k = e / H, c = 2 * (e - k * H);
+            double2 v = make_double2(0.0, 0.0);
+            if (c < ncol) { v = __ldcs(reinterpret_cast<const double2*>(fsrc + (long)k * plane + c)); v.x *= scale; v.y *= scale; }
+            *reinterpret_cast<double2*>(A + k * CT + c) = v;
         }
-        Phi[e] = phi;
-    }
-    __syncthreads();
-    for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-        int k = e / CT, c = e - k * CT;
-        if (c < ncol) {
-            double lo = k > 0 ? Phi[e - CT] : 0.0;
-            fb[(long)k * plane + c] = A[e] + (lo - Phi[e]);      // eq. (38)
+        __syncthreads();
+        for (int wi = threadIdx.x; wi < CT * P.nseg; wi += V_THREADS) {
+            const int seg = wi / CT, c = wi - seg * CT;
+            if (c < ncol) {
+                const int col = c0 + c;
+                const int k1 = col / P.nv2, k2 = col - k1 * P.nv2;
+                const double s0 = t0 + t2 * k1 + t3 * k2;
+                const int a = seg * seglen, b = min(a + seglen, N);
+                double* o = fb + c;
+                march_cells<LIM>(A + c, CT, N, a, b, s0, t1, finf,
+                                 [&](int i, double v) { __stcs(o + (long)i * plane, v); });
+            }
         }
+        __syncthreads();
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// a5 + a6: vy sweep then vz sweep on a tile of PT contiguous i_vx planes.
+// a5 + a6: vy sweep then vz sweep on a tile of PT contiguous i_vx planes.  Shared layout of a buffer:
+// cell (p, y, z) at OFF + p PS + y RS + z with RS = N2 + 3 (odd: threads that march neighbouring z
+// lines hit distinct banks), PS = (N1 + 3) RS, OFF = 3 RS + 3; everything that is not a cell is zero and
+// serves as the padding of the lines in both directions.  vy: A -> Bf; vz: Bf -> A; A -> global.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) vsweep_yz_kernel(VParams P) {
+template <int LIM>
+__global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
     extern __shared__ double sm[];
-    const int N1 = P.nv1, N2 = P.nv2;
+    const int N1 = P.nv1, N2 = P.nv2, H2 = N2 >> 1;
     const int plane = N1 * N2;
-    const int cell = P.cell0 + blockIdx.x / P.ntile;
-    const int p0 = (blockIdx.x % P.ntile) * P.ct;
-    const int np = min(P.ct, P.nv0 - p0);
-    const int tot = np * plane;
+    const int RS = N2 + 3, PS = (N1 + 3) * RS, OFF = 3 * RS + 3;
+    const int BUF = (OFF + P.ct * PS + 1) & ~1;
     double* A = sm;
-    double* Phi = sm + (long)P.ct * plane;
-    double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
-    const double* T = P.table + (long)cell * TAB;
-    for (int e = threadIdx.x; e < tot; e += blockDim.x) A[e] = fb[e];
+    double* Bf = sm + BUF;
+    for (int e = threadIdx.x; e < 2 * BUF; e += V_THREADS) sm[e] = 0.0;
     __syncthreads();
-    {   // vy: line along i_vy (stride N2); transverse (i_vx, i_vz)
-        const double t0 = T[4], t1 = T[5], t2 = T[6], t3 = T[7], finf = T[13];
-        for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-            int p = e / plane, r = e - p * plane;
-            int k = r / N2, z = r - k * N2;
-            double phi = 0.0;
-            if (k < N1 - 1) {
-                double sigma = t0 + t1 * (k + 1) + t2 * (p0 + p) + t3 * z;
-                phi = face_flux(A, p * plane + z, N2, N1, k, sigma, finf, P.limiter);
+    const unsigned mH2 = (unsigned)(0xFFFFFFFFull / (unsigned)H2);       // floor(2^32 / H2) or one less
+    for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x) {
+        const int cell = P.cell0 + tile / P.ntile;
+        const int p0 = (tile % P.ntile) * P.ct;
+        const int np = min(P.ct, P.nv0 - p0);
+        double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
+        const double* T = P.table + (long)cell * TAB;
+        const int nrow = np * N1;
+        for (int e = threadIdx.x; e < nrow * H2; e += V_THREADS) {
+            unsigned row = __umulhi((unsigned)e, mH2);
+            int z2 = e - (int)row * H2;
+            if (z2 >= H2) { z2 -= H2; ++row; }
+            if (z2 >= H2) { z2 -= H2; ++row; }
+            const int p = (int)row / N1, y = (int)row - p * N1;
+            const double2 v = __ldcs(reinterpret_cast<const double2*>(fb) + e);
+            double* d = A + OFF + p * PS + y * RS + 2 * z2;
+            d[0] = v.x; d[1] = v.y;
+        }
+        __syncthreads();
+        {   // vy: line along i_vy (stride RS); transverse (i_vx, i_vz); thread index runs along z
+            const double t0 = T[4], t1 = T[5], t2 = T[6], t3 = T[7], finf = T[13];
+            const int seglen = (N1 + P.nseg - 1) / P.nseg;
+            const int nl = np * N2;
+            for (int wi = threadIdx.x; wi < nl * P.nseg; wi += V_THREADS) {
+                const int seg = wi / nl, l = wi - seg * nl;
+                const int p = l / N2, z = l - p * N2;
+                const double s0 = t0 + t2 * (p0 + p) + t3 * z;
+                const int a = seg * seglen, b = min(a + seglen, N1);
+                double* o = Bf + OFF + p * PS + z;
+                march_cells<LIM>(A + OFF + p * PS + z, RS, N1, a, b, s0, t1, finf,
+                                 [&](int i, double v) { o[i * RS] = v; });
             }
-            Phi[e] = phi;
         }
         __syncthreads();
-        for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-            int r = e % plane;
-            int k = r / N2;
-            double lo = k > 0 ? Phi[e - N2] : 0.0;
-            A[e] = A[e] + (lo - Phi[e]);
-        }
-        __syncthreads();
-    }
-    {   // vz: contiguous lines; transverse (i_vx, i_vy)
-        const double t0 = T[8], t1 = T[9], t2 = T[10], t3 = T[11], finf = T[14];
-        for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-            int p = e / plane, r = e - p * plane;
-            int y = r / N2, k = r - y * N2;
-            double phi = 0.0;
-            if (k < N2 - 1) {
-                double sigma = t0 + t1 * (k + 1) + t2 * (p0 + p) + t3 * y;
-                phi = face_flux(A, e - k, 1, N2, k, sigma, finf, P.limiter);
+        {   // vz: contiguous lines; transverse (i_vx, i_vy); thread index runs along y (stride RS, odd)
+            const double t0 = T[8], t1 = T[9], t2 = T[10], t3 = T[11], finf = T[14];
+            const int seglen = (N2 + P.nseg - 1) / P.nseg;
+            const int nl = np * N1;
+            for (int wi = threadIdx.x; wi < nl * P.nseg; wi += V_THREADS) {
+                const int seg = wi / nl, l = wi - seg * nl;
+                const int p = l / N1, y = l - p * N1;
+                const double s0 = t0 + t2 * (p0 + p) + t3 * y;
+                const int a = seg * seglen, b = min(a + seglen, N2);
+                double* o = A + OFF + p * PS + y * RS;
+                march_cells<LIM>(Bf + OFF + p * PS + y * RS, 1, N2, a, b, s0, t1, finf,
+                                 [&](int i, double v) { o[i] = v; });
             }
-            Phi[e] = phi;
         }
         __syncthreads();
-        for (int e = threadIdx.x; e < tot; e += blockDim.x) {
-            int k = e % N2;
-            double lo = k > 0 ? Phi[e - 1] : 0.0;
-            fb[e] = A[e] + (lo - Phi[e]);
+        for (int e = threadIdx.x; e < nrow * H2; e += V_THREADS) {
+            unsigned row = __umulhi((unsigned)e, mH2);
+            int z2 = e - (int)row * H2;
+            if (z2 >= H2) { z2 -= H2; ++row; }
+            if (z2 >= H2) { z2 -= H2; ++row; }
+            const int p = (int)row / N1, y = (int)row - p * N1;
+            const double* d = A + OFF + p * PS + y * RS + 2 * z2;
+            __stcs(reinterpret_cast<double2*>(fb) + e, make_double2(d[0], d[1]));
         }
+        __syncthreads();
     }
 }
 
-static int g_smem_set = 0;
+static int g_occ_x[2] = {0, 0}, g_occ_yz[2] = {0, 0};
+static size_t g_occ_x_smem[2] = {0, 0}, g_occ_yz_smem[2] = {0, 0};
+constexpr size_t V_SMEM_MAX = 200 * 1024;
+
+template <class K>
+static int resident_ctas(K kernel, size_t smem, int& cache, size_t& cache_smem) {
+    if (cache > 0 && cache_smem == smem) return cache;
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V_SMEM_MAX);
+    int per_sm = 0, dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, V_THREADS, smem);
+    if (per_sm < 1) per_sm = 1;
+    cache = per_sm * sms;
+    cache_smem = smem;
+    return cache;
+}
 
 int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows) {
     if (nrows <= 0) return VLASOV_OK;
-    if (!g_smem_set) {
-        cudaFuncSetAttribute(vsweep_x_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        cudaFuncSetAttribute(vsweep_yz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        g_smem_set = 1;
-    }
     VParams P;
     P.f = f; P.table = c->table; P.S = s.nvtot;
     P.nv0 = s.nv[0]; P.nv1 = s.nv[1]; P.nv2 = s.nv[2];
     P.cell0 = row0 * c->G.nx;
-    P.limiter = c->G.limiter;
+    const int lim = c->G.limiter ? 1 : 0;
     const int ncell = nrows * c->G.nx;
     const int plane = s.nv[1] * s.nv[2];
     {
         int ct = 128;
-        while (ct > 32 && (size_t)2 * s.nv[0] * ct * 8 > 96 * 1024) ct >>= 1;
-        if (ct > plane) ct = plane;
+        while (ct > 32 && ((size_t)(s.nv[0] + 6) * ct * 8 > 48 * 1024 || ct / 2 >= plane)) ct >>= 1;
         P.ct = ct;
-        size_t smem = (size_t)2 * s.nv[0] * ct * 8;
-        if (smem > 200 * 1024) return VLASOV_EINVAL;
+        const size_t smem = (size_t)(s.nv[0] + 6) * ct * 8;
+        if (smem > V_SMEM_MAX) return VLASOV_EINVAL;
         P.ntile = (plane + ct - 1) / ct;
+        P.ntot = P.ntile * ncell;
+        P.nseg = V_THREADS / ct; if (P.nseg < 1) P.nseg = 1; if (P.nseg > s.nv[0]) P.nseg = s.nv[0];
+        auto k = lim ? vsweep_x_kernel<1> : vsweep_x_kernel<0>;
+        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim], g_occ_x_smem[lim]));
         Launch L(c, K_VSWEEP_X);
-        vsweep_x_kernel<<<(unsigned)((long)P.ntile * ncell), 256, smem, c->stream>>>(P);
+        k<<<grid, V_THREADS, smem, c->stream>>>(P);
     }
     {
-        int pt = (int)((32 * 1024) / ((size_t)plane * 8));
+        const size_t rs = s.nv[2] + 3, ps = (s.nv[1] + 3) * rs, off = 3 * rs + 3;
+        int pt = (int)((44 * 1024 / 8 - off) / ps);
         if (pt < 1) pt = 1;
         if (pt > s.nv[0]) pt = s.nv[0];
+        while (pt > 1 && s.nv[0] % pt) --pt;            // equal tiles
         P.ct = pt;
-        size_t smem = (size_t)2 * pt * plane * 8;
-        if (smem > 200 * 1024) return VLASOV_EINVAL;
+        const size_t buf = (off + pt * ps + 1) & ~(size_t)1;
+        const size_t smem = 2 * buf * 8;
+        if (smem > V_SMEM_MAX) return VLASOV_EINVAL;
         P.ntile = (s.nv[0] + pt - 1) / pt;
+        P.ntot = P.ntile * ncell;
+        const int nl = pt * min(s.nv[1], s.nv[2]);
+        P.nseg = V_THREADS / nl; if (P.nseg < 1) P.nseg = 1;
+        if (P.nseg > min(s.nv[1], s.nv[2]) / 4) P.nseg = max(1, min(s.nv[1], s.nv[2]) / 4);
+        auto k = lim ? vsweep_yz_kernel<1> : vsweep_yz_kernel<0>;
+        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim], g_occ_yz_smem[lim]));
         Launch L(c, K_VSWEEP_YZ);
-        vsweep_yz_kernel<<<(unsigned)((long)P.ntile * ncell), 256, smem, c->stream>>>(P);
+        k<<<grid, V_THREADS, smem, c->stream>>>(P);
     }
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
