@@ -121,72 +121,122 @@ int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const
 // R7), so the three reads around the foot cell need no bounds checks.  eq. (46) for sigma >= 0, eq. (47)
 // (sum repaired, R5) for sigma < 0: the same expression on the mirrored line.
 // ------------------------------------------------------------------------------------------------
-// Limited slopes with a warp-level fast path: where no lane's slope needs limiting (|d+-| <= min(2 f_j,
-// 2 (f_inf - f_j)), the bulk of a smooth distribution) eqs. (43), (44) give eps = 1 and the clamps are
-// skipped.  fp64 min/max cost ~6 instructions each on sm_100a (DSETP + selects), so this matters.
+// ---- shared memory by 32-bit address (keeps the window base out of the inner loops) ----------------
+__device__ __forceinline__ double lds(unsigned a) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v)); }
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// max(x, 0) on the bit pattern (no NaN fix-up code): x if its sign bit is clear, else +0.
+__device__ __forceinline__ double relu_bits(double x) {
+    const int h = __double2hiint(x);
+    const int m = ~(h >> 31);
+    return __hiloint2double(h & m, __double2loint(x) & m);
+}
+
+// Limited slopes eps+ d+, eps- d- of eqs. (43), (44) (R6) in the division-free clamp form
+//     eps+ d+ = clamp(d+, -max(0,Bv), max(0,A)),  eps- d- = clamp(d-, -max(0,A), max(0,Bv)),  A = 2 f0, Bv = 2 (f_inf - f0)
+// written in sign/magnitude: |eps d| = min(|d|, bound picked by the sign of d).  fp64 issue slots are the
+// scarce resource on this path, so the test "does any lane of the warp
+// need limiting at all" is done on the HIGH WORDS of the doubles in the integer pipe: for non-negative
+// doubles the IEEE order is the integer order, so
+//     hi(|d|) < min(hi(2 f0), hi(2 (f_inf - f0)))   ==>   |d| < min(2 f0, 2 (f_inf - f0))   ==>   eps = 1.
+// The test is conservative (ties and negative bounds fall through to the exact clamps); hi(2 x) is
+// hi(x) + 2^20 (exponent + 1; the denormal corner only ever errs by < 1e-307).
 template <int LIM>
 __device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, double finf, double& sp, double& sm) {
     const double dp = fp - f0, dm = f0 - fm;
     sp = dp; sm = dm;
     if (LIM) {
-        const double A = f0 + f0;
-        const double Bv = fma(-2.0, f0, finf + finf);
-        const double m = A < Bv ? A : Bv;
-        const bool need = !(fabs(dp) <= m && fabs(dm) <= m);
+        const double g = finf - f0;
+        const int hb = min(__double2hiint(f0), __double2hiint(g)) + 0x00100000;
+        const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
+        const bool need = max(hp, hm) >= hb;
         if (__any_sync(__activemask(), need)) {
-            const double hiA = A > 0.0 ? A : 0.0, hiB = Bv > 0.0 ? Bv : 0.0;
-            sp = dp < -hiB ? -hiB : dp; sp = sp > hiA ? hiA : sp;
-            sm = dm < -hiA ? -hiA : dm; sm = sm > hiB ? hiB : sm;
+            const double hiA = relu_bits(f0 + f0), hiB = relu_bits(g + g);
+            const bool pneg = __double2hiint(dp) < 0, mneg = __double2hiint(dm) < 0;
+            const double bp = pneg ? hiB : hiA;
+            const double bm = mneg ? hiA : hiB;
+            const double ap = __hiloint2double(hp, __double2loint(dp));      // |d+|
+            const double am = __hiloint2double(hm, __double2loint(dm));      // |d-|
+            const double mp = ap < bp ? ap : bp;
+            const double mm = am < bm ? am : bm;
+            sp = __hiloint2double(__double2hiint(mp) | (__double2hiint(dp) & 0x80000000), __double2loint(mp));
+            sm = __hiloint2double(__double2hiint(mm) | (__double2hiint(dm) & 0x80000000), __double2loint(mm));
         }
     }
 }
 
+// Flux through face k (between cells k-1 and k, 1 <= k <= N-1) of a ZERO-PADDED line in shared memory:
+// L = shared byte address of cell 0, st8 = stride in bytes, cells -3..-1 and N..N+2 hold zeros (f = 0
+// outside the box, R7).  eq. (46) for sigma >= 0, eq. (47) (sum repaired, R5) for sigma < 0: the same
+// expression on the mirrored line.  floor() by a round-down add of 1.5 * 2^52: n sits in the low word,
+// alpha = |sigma| - n in [0,1).
 template <int LIM>
-__device__ __forceinline__ double face_flux_pad(const double* __restrict__ L, int st, int N, int k, double sigma,
-                                                double finf) {
-    const bool pos = sigma >= 0.0;
-    int n; double b;
-    split_shift(fabs(sigma), n, b);
-    const int u = pos ? 1 : -1;
-    int j = pos ? k - 1 - n : k + n;                 // foot cell
-    const int m0 = pos ? j + 1 : k;                  // the n whole cells between foot cell and face
-    const int lo = max(m0, 0), hi = min(m0 + n, N);
+__device__ __forceinline__ double face_flux_pad(unsigned L, int st8, int N, int k, double sigma, double finf) {
+    const double M = 6755399441055744.0;
+    const double as = fabs(sigma);
+    const double r = __dadd_rd(as, M);
+    const int n = __double2loint(r);
+    const double b = as - (r - M);
+    const int sg = __double2hiint(sigma) >> 31;      // 0: sigma >= 0, -1: sigma < 0
+    int j = k + (n ^ ~sg);                           // foot cell: k-1-n | k+n
     double sum = 0.0;
+    if (n > 0) {                                     // the n whole cells between foot cell and face
+        const int m0 = k - (n & ~sg);                // k-n | k
+        const int lo = max(m0, 0), hi = min(m0 + n, N);
+        unsigned am = L + lo * st8;
 #pragma unroll 1
-    for (int m = lo; m < hi; ++m) sum += L[m * st];
+        for (int m = lo; m < hi; ++m) { sum += lds(am); am += st8; }
+    }
     j = min(max(j, -2), N + 1);
-    const double* pj = L + j * st;
-    const int ust = pos ? st : -st;
-    const double f0 = pj[0];
-    const double fm = pj[-ust];
-    const double fp = pj[ust];
+    const unsigned aj = L + j * st8;
+    const int ust8 = (st8 ^ sg) - sg;                // +st8 | -st8
+    const double f0 = lds(aj);
+    const double fm = lds(aj - ust8);
+    const double fp = lds(aj + ust8);
     double sp, sm;
     slopes_fast<LIM>(fm, f0, fp, finf, sp, sm);
-    const double omb = 1.0 - b;
-    const double t = omb * (1.0 / 6.0);
-    const double c1 = t * (2.0 - b);
-    const double c2 = t * (1.0 + b);
-    const double phi = sum + b * (f0 + c1 * sp + c2 * sm);
+    // alpha [ f0 + (1-a)(2-a)/6 sp + (1-a)(1+a)/6 sm ]: the two weights as polynomials in alpha
+    const double b2 = b * b;
+    const double c1 = fma(b2, 1.0 / 6.0, fma(b, -0.5, 1.0 / 3.0));
+    const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+    const double phi = fma(b, fma(c1, sp, fma(c2, sm, f0)), sum);
     // phi for sigma >= 0, -phi otherwise: flip the sign bit with sigma's
-    const int hi32 = __double2hiint(phi) ^ (__double2hiint(sigma) & 0x80000000);
-    return __hiloint2double(hi32, __double2loint(phi));
+    return __hiloint2double(__double2hiint(phi) ^ (sg & 0x80000000), __double2loint(phi));
 }
 
 // One thread remaps cells [a, b) of one line: flux per face, eq. (38) per cell.  sigma of face k is
-// s0 + s1 k.  put(i, value) stores the new cell average.
-template <int LIM, class Put>
-__device__ __forceinline__ void march_cells(const double* __restrict__ L, int st, int N, int a, int b, double s0,
-                                            double s1, double finf, Put put) {
-    double kd = (double)a;
-    double phi_lo = a > 0 ? face_flux_pad<LIM>(L, st, N, a, fma(s1, kd, s0), finf) : 0.0;
+// s0 + s1 k (accumulated).  out.put(value) stores the new average of the next cell (a, a+1, ...).
+template <int LIM, class Out>
+__device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
+                                            double finf, Out& out) {
+    double sig = fma(s1, (double)a, s0);
+    double phi_lo = a > 0 ? face_flux_pad<LIM>(L, st8, N, a, sig, finf) : 0.0;
+    unsigned ci = L + a * st8;
+    const int bi = b < N ? b : N - 1;                // faces a+1 .. bi are interior
 #pragma unroll 2
-    for (int i = a; i < b; ++i) {
-        kd += 1.0;
-        const double phi_hi = i + 1 < N ? face_flux_pad<LIM>(L, st, N, i + 1, fma(s1, kd, s0), finf) : 0.0;
-        put(i, L[i * st] + (phi_lo - phi_hi));       // eq. (38): f + (Phi_{i-1/2} - Phi_{i+1/2})
+    for (int k = a + 1; k <= bi; ++k) {
+        sig += s1;
+        const double phi_hi = face_flux_pad<LIM>(L, st8, N, k, sig, finf);
+        out.put(lds(ci) + (phi_lo - phi_hi));        // eq. (38): f + (Phi_{i-1/2} - Phi_{i+1/2})
+        ci += st8;
         phi_lo = phi_hi;
     }
+    if (b == N) out.put(lds(ci) + phi_lo);           // zero flux through the upper box face (R7)
 }
+
+struct OutShared {       // consecutive cells of a line in shared memory
+    unsigned a; int st8;
+    __device__ __forceinline__ void put(double v) { sts(a, v); a += st8; }
+};
+struct OutGlobal {       // consecutive cells of a line in global memory (streaming store)
+    double* p; long st;
+    __device__ __forceinline__ void put(double v) { __stcs(p, v); p += st; }
+};
 
 // q = e / d, r = e % d with m = floor((2^32 - 1) / d): the estimate is at most 2 short.
 __device__ __forceinline__ void fast_divmod(unsigned e, unsigned d, unsigned m, unsigned& q, unsigned& r) {
@@ -245,9 +295,8 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_x_kernel(VParams P) {
                 const int k1 = col / P.nv2, k2 = col - k1 * P.nv2;
                 const double s0 = t0 + t2 * k1 + t3 * k2;
                 const int a = seg * seglen, b = min(a + seglen, N);
-                double* o = fb + c;
-                march_cells<LIM>(A + c, CT, N, a, b, s0, t1, finf,
-                                 [&](int i, double v) { __stcs(o + (long)i * plane, v); });
+                OutGlobal o{fb + c + (long)a * plane, (long)plane};
+                march_cells<LIM>(smem_addr(A + c), CT * 8, N, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
@@ -296,9 +345,8 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
                 const int p = l / N2, z = l - p * N2;
                 const double s0 = t0 + t2 * (p0 + p) + t3 * z;
                 const int a = seg * seglen, b = min(a + seglen, N1);
-                double* o = Bf + OFF + p * PS + z;
-                march_cells<LIM>(A + OFF + p * PS + z, RS, N1, a, b, s0, t1, finf,
-                                 [&](int i, double v) { o[i * RS] = v; });
+                OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
+                march_cells<LIM>(smem_addr(A + OFF + p * PS + z), RS * 8, N1, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
@@ -311,9 +359,8 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
                 const int p = l / N1, y = l - p * N1;
                 const double s0 = t0 + t2 * (p0 + p) + t3 * y;
                 const int a = seg * seglen, b = min(a + seglen, N2);
-                double* o = A + OFF + p * PS + y * RS;
-                march_cells<LIM>(Bf + OFF + p * PS + y * RS, 1, N2, a, b, s0, t1, finf,
-                                 [&](int i, double v) { o[i] = v; });
+                OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
+                march_cells<LIM>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
