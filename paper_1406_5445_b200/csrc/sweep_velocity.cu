@@ -128,6 +128,10 @@ __device__ __forceinline__ double lds(unsigned a) {
     return v;
 }
 __device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v)); }
+__device__ __forceinline__ void cp_async8(unsigned dst, const double* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 __device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 // max(x, 0) on the bit pattern (no NaN fix-up code): x if its sign bit is clear, else +0.
@@ -255,7 +259,8 @@ struct VParams {
     int ct;           // columns per tile (vx kernel) / planes per tile (vyz kernel)
     int ntile;        // tiles per spatial cell
     int ntot;         // tiles of this launch
-    int nseg;         // threads per line
+    int nseg;         // threads per line (vx kernel; vy lines of the vyz kernel)
+    int nseg2;        // threads per vz line
 };
 
 constexpr int V_THREADS = 256;
@@ -320,20 +325,31 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
     double* Bf = sm + BUF;
     for (int e = threadIdx.x; e < 2 * BUF; e += V_THREADS) sm[e] = 0.0;
     __syncthreads();
-    const unsigned mN2 = (unsigned)(0xFFFFFFFFull / (unsigned)N2);       // floor(2^32 / N2) or one less
-    const unsigned mN1 = (unsigned)(0xFFFFFFFFull / (unsigned)N1);
+    // cell e = threadIdx.x of a tile sits at (pp, y, z); stepping e by V_THREADS moves it by (dpp, dy, dz) plus carries
+    const unsigned sA = smem_addr(A);
+    const int z_init = threadIdx.x % N2, row_init = threadIdx.x / N2;
+    const int y_init = row_init % N1;
+    const unsigned so_init = OFF + (row_init / N1) * PS + y_init * RS + z_init;
+    const int dz = V_THREADS % N2, drow = V_THREADS / N2;
+    const int dy = drow % N1;
+    const unsigned dso = dz + dy * RS + (drow / N1) * PS;
     for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x) {
         const int cell = P.cell0 + tile / P.ntile;
         const int p0 = (tile % P.ntile) * P.ct;
         const int np = min(P.ct, P.nv0 - p0);
         double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
         const double* T = P.table + (long)cell * TAB;
-        const int nrow = np * N1;
-        for (int e = threadIdx.x; e < nrow * N2; e += V_THREADS) {
-            unsigned row, z, pp, y;
-            fast_divmod((unsigned)e, (unsigned)N2, mN2, row, z);
-            fast_divmod(row, (unsigned)N1, mN1, pp, y);
-            A[OFF + pp * PS + y * RS + z] = __ldcs(fb + e);
+        const int ncellt = np * plane;
+        {   // global -> A by 8-byte cp.async; (pp, y, z) of e = threadIdx.x + i V_THREADS advanced by carries
+            int z = z_init, y = y_init;
+            unsigned so = so_init;
+            for (int e = threadIdx.x; e < ncellt; e += V_THREADS) {
+                cp_async8(sA + so * 8, fb + e);
+                z += dz; y += dy; so += dso;
+                if (z >= N2) { z -= N2; so += RS - N2; ++y; }
+                if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+            }
+            cp_async_wait_all();
         }
         __syncthreads();
         {   // vy: line along i_vy (stride RS); transverse (i_vx, i_vz); thread index runs along z
@@ -352,9 +368,9 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
         __syncthreads();
         {   // vz: contiguous lines; transverse (i_vx, i_vy); thread index runs along y (stride RS, odd)
             const double t0 = T[8], t1 = T[9], t2 = T[10], t3 = T[11], finf = T[14];
-            const int seglen = (N2 + P.nseg - 1) / P.nseg;
+            const int seglen = (N2 + P.nseg2 - 1) / P.nseg2;
             const int nl = np * N1;
-            for (int wi = threadIdx.x; wi < nl * P.nseg; wi += V_THREADS) {
+            for (int wi = threadIdx.x; wi < nl * P.nseg2; wi += V_THREADS) {
                 const int seg = wi / nl, l = wi - seg * nl;
                 const int p = l / N1, y = l - p * N1;
                 const double s0 = t0 + t2 * (p0 + p) + t3 * y;
@@ -364,11 +380,15 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
             }
         }
         __syncthreads();
-        for (int e = threadIdx.x; e < nrow * N2; e += V_THREADS) {
-            unsigned row, z, pp, y;
-            fast_divmod((unsigned)e, (unsigned)N2, mN2, row, z);
-            fast_divmod(row, (unsigned)N1, mN1, pp, y);
-            __stcs(fb + e, A[OFF + pp * PS + y * RS + z]);
+        {
+            int z = z_init, y = y_init;
+            unsigned so = so_init;
+            for (int e = threadIdx.x; e < ncellt; e += V_THREADS) {
+                __stcs(fb + e, lds(sA + so * 8));
+                z += dz; y += dy; so += dso;
+                if (z >= N2) { z -= N2; so += RS - N2; ++y; }
+                if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+            }
         }
         __syncthreads();
     }
@@ -417,7 +437,8 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
     }
     {
         const size_t rs = s.nv[2] + 3, ps = (s.nv[1] + 3) * rs, off = 3 * rs + 3;
-        int pt = (int)((44 * 1024 / 8 - off) / ps);
+        // segments of about 8 cells per thread, about V_THREADS threads per tile: small tiles, many CTAs per SM
+        int pt = (8 * V_THREADS) / plane;
         if (pt < 1) pt = 1;
         if (pt > s.nv[0]) pt = s.nv[0];
         while (pt > 1 && s.nv[0] % pt) --pt;            // equal tiles
@@ -427,9 +448,8 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (smem > V_SMEM_MAX) return VLASOV_EINVAL;
         P.ntile = (s.nv[0] + pt - 1) / pt;
         P.ntot = P.ntile * ncell;
-        const int nl = pt * min(s.nv[1], s.nv[2]);
-        P.nseg = V_THREADS / nl; if (P.nseg < 1) P.nseg = 1;
-        if (P.nseg > min(s.nv[1], s.nv[2]) / 4) P.nseg = max(1, min(s.nv[1], s.nv[2]) / 4);
+        P.nseg = (s.nv[1] + 7) / 8;
+        P.nseg2 = (s.nv[2] + 7) / 8;
         auto k = lim ? vsweep_yz_kernel<1> : vsweep_yz_kernel<0>;
         const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim], g_occ_yz_smem[lim]));
         Launch L(c, K_VSWEEP_YZ);
