@@ -145,10 +145,17 @@ int vlasov_cycle_host(vlasov_ctx* ctx, double dt, int nsub, double* E_host, doub
  * clears the record. */
 enum {
     VLASOV_KIND_SWEEP_X = 0, VLASOV_KIND_SWEEP_Y, VLASOV_KIND_TABLE, VLASOV_KIND_VSWEEP_X, VLASOV_KIND_VSWEEP_YZ,
-    VLASOV_KIND_MOMENTS, VLASOV_KIND_GHOST_TABLE, VLASOV_KIND_CURRENT, VLASOV_KIND_MAXWELL, VLASOV_KIND_COUNT
+    VLASOV_KIND_MOMENTS, VLASOV_KIND_GHOST_TABLE, VLASOV_KIND_CURRENT, VLASOV_KIND_MAXWELL, VLASOV_KIND_SWEEP_XY,
+    VLASOV_KIND_COUNT
 };
 int vlasov_timing_enable(vlasov_ctx* ctx, int on);
 int vlasov_timing_read(vlasov_ctx* ctx, double* ms_by_kind, int64_t* count_by_kind, int nkinds);
+
+/* Execution options (results stay within the parity tolerance either way).
+ * VLASOV_OPT_FUSE_XY (default 1): run each spatial stage (x/2 y/2, y/2 x/2) as ONE fused pass over f when every
+ * shift of the stage is below one cell; 0 = always the general one-direction kernels.  Errors: EINVAL. */
+enum { VLASOV_OPT_FUSE_XY = 1 };
+int vlasov_set_option(vlasov_ctx* ctx, int option, int value);
 
 /* Tell the library the caller wrote into an f buffer itself (drops the kept moments). */
 int vlasov_touch(vlasov_ctx* ctx);

@@ -16,10 +16,11 @@ ORDER_XVX, ORDER_VXV = 0, 1
 STAGE_X1, STAGE_V, STAGE_X2, STAGE_GHOST, STAGE_MOMENTS, STAGE_ALL = 1, 2, 4, 8, 16, 31
 
 EXPORTS = ["vlasov_scratch_bytes", "vlasov_init", "vlasov_set_boundary", "vlasov_step", "vlasov_step_host",
-           "vlasov_moments", "vlasov_current", "vlasov_maxwell", "vlasov_touch", "vlasov_check",
+           "vlasov_moments", "vlasov_current", "vlasov_maxwell", "vlasov_touch", "vlasov_set_option", "vlasov_check",
            "vlasov_launch_count", "vlasov_free", "vlasov_strerror", "vlasov_cycle", "vlasov_cycle_host",
            "vlasov_timing_enable", "vlasov_timing_read"]
-KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell"]
+OPT_FUSE_XY = 1
+KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy"]
 
 
 class vlasov_species(C.Structure):
@@ -77,6 +78,8 @@ def lib():
         L.vlasov_timing_enable.argtypes = [vp, C.c_int]
         L.vlasov_timing_read.restype = C.c_int
         L.vlasov_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
+        L.vlasov_set_option.restype = C.c_int
+        L.vlasov_set_option.argtypes = [vp, C.c_int, C.c_int]
         L.vlasov_touch.restype = C.c_int
         L.vlasov_touch.argtypes = [vp]
         L.vlasov_check.restype = C.c_int
@@ -200,6 +203,9 @@ class Context:
         cnt = (C.c_int64 * n)()
         _chk(lib().vlasov_timing_read(self.h, ms, cnt, n), "vlasov_timing_read")
         return {KINDS[k]: (float(ms[k]), int(cnt[k])) for k in range(n)}
+
+    def vlasov_set_option(self, option, value):
+        _chk(lib().vlasov_set_option(self.h, int(option), int(value)), "vlasov_set_option")
 
     def vlasov_touch(self):
         _chk(lib().vlasov_touch(self.h), "vlasov_touch")

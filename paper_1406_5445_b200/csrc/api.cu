@@ -46,18 +46,32 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         if (G.bc_lo == VLASOV_BC_FLUID) { e = launch_ghost_fill(c, s, s.f, 0); if (e) return e; }
         if (G.bc_hi == VLASOV_BC_FLUID) { e = launch_ghost_fill(c, s, s.f, 1); if (e) return e; }
     }
+    // cur: where this species' f lives right now.  The general spatial stage is f -> pong -> f; the fused
+    // stage is ONE pass cur -> other, so the buffers swap roles; an odd number of fused stages in one call
+    // is settled by a copy back into the caller's buffer at the end.
+    double* cur = s.f;
     auto space = [&](double dts, bool x_first) -> int {
         int r;
-        if (x_first) {
-            r = launch_sweep_x(c, s, s.f, c->pong, dts); if (r) return r;
-            return launch_sweep_y(c, s, c->pong, s.f, dts);
+        double* other = cur == s.f ? c->pong : s.f;
+        if (c->fuse_xy && fused_xy_applicable(c, s, dts)) {
+            r = launch_sweep_xy(c, s, cur, other, dts, x_first ? 1 : 0); if (r) return r;
+            if (G.g > 0) {      // x sweeps update ghost rows too, y sweeps never do (R16)
+                r = launch_sweep_x_rows(c, s, cur, other, dts, 0, G.g); if (r) return r;
+                r = launch_sweep_x_rows(c, s, cur, other, dts, G.g + G.ny, G.g); if (r) return r;
+            }
+            cur = other;
+            return VLASOV_OK;
         }
-        r = launch_sweep_y(c, s, s.f, c->pong, dts); if (r) return r;
-        return launch_sweep_x(c, s, c->pong, s.f, dts);
+        if (x_first) {
+            r = launch_sweep_x(c, s, cur, other, dts); if (r) return r;
+            return launch_sweep_y(c, s, other, cur, dts);
+        }
+        r = launch_sweep_y(c, s, cur, other, dts); if (r) return r;
+        return launch_sweep_x(c, s, other, cur, dts);
     };
     auto velocity = [&](double dtv) -> int {
         int r = launch_lorentz_table(c, s, E, B, dtv); if (r) return r;
-        return launch_vsweeps(c, s, s.f, 0, G.nyg);      // ghost rows too (R16)
+        return launch_vsweeps(c, s, cur, 0, G.nyg);      // ghost rows too (R16)
     };
     if (c->order == VLASOV_ORDER_XVX) {
         if (stages & VLASOV_STAGE_X1) { e = space(dt / 2.0, true); if (e) return e; }
@@ -67,6 +81,10 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         if (stages & VLASOV_STAGE_X1) { e = velocity(dt / 2.0); if (e) return e; }
         if (stages & VLASOV_STAGE_V) { e = space(dt, true); if (e) return e; }
         if (stages & VLASOV_STAGE_X2) { e = velocity(dt / 2.0); if (e) return e; }
+    }
+    if (cur != s.f) {
+        VL_CUDA_OK(cudaMemcpyAsync(s.f, cur, (size_t)G.nyg * G.nx * s.nvtot * 8, cudaMemcpyDeviceToDevice, c->stream));
+        c->launches++;
     }
     if (stages & VLASOV_STAGE_MOMENTS) {
         const long ncell = (long)G.nyg * G.nx;
@@ -149,6 +167,7 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     c->errflag = (int*)(base + C.err);
     c->timing = 0; c->nrec = 0; c->ev0 = c->ev1 = nullptr; c->rec_kind = nullptr;
     c->mom_valid = 0;
+    c->fuse_xy = 1;
     c->launches = 0;
     c->h_err = nullptr;
     if (cudaMallocHost((void**)&c->h_err, sizeof(int)) != cudaSuccess) { delete c; return VLASOV_ECUDA; }
@@ -284,6 +303,12 @@ int vlasov_maxwell(vlasov_ctx* c, double dt, int nsub, double* E_dev, double* B_
                    double* Bavg_dev) {
     if (!c || nsub <= 0 || !E_dev || !B_dev || !J_dev) return VLASOV_EINVAL;
     return launch_maxwell(c, dt, nsub, E_dev, B_dev, J_dev, Bavg_dev);
+}
+
+int vlasov_set_option(vlasov_ctx* c, int option, int value) {
+    if (!c) return VLASOV_EINVAL;
+    if (option == VLASOV_OPT_FUSE_XY) { c->fuse_xy = value ? 1 : 0; return VLASOV_OK; }
+    return VLASOV_EINVAL;
 }
 
 int vlasov_touch(vlasov_ctx* c) {

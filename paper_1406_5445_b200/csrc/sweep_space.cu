@@ -25,6 +25,7 @@ struct SpaceParams {
     double finf;
     int limiter;
     int bc_lo, bc_hi;
+    int row0;          // x sweep: first ghost-inclusive row of this launch
     int* err;
 };
 
@@ -82,7 +83,7 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     const long v = chunk * VEC;
     const int ivx = (int)(v / ((long)P.nv1 * P.nv2));
     const int ivy = (int)((v / P.nv2) % P.nv1);
-    const int other = blockIdx.y;           // x sweep: ghost-inclusive row; y sweep: ix
+    const int other = P.row0 + blockIdx.y;  // x sweep: ghost-inclusive row; y sweep: ix
     const double* base;
     double* obase;
     long mir = 0;
@@ -149,7 +150,8 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     if (bad) atomicCAS(P.err, 0, VLASOV_ESHIFT);
 }
 
-static int launch_space(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int axis) {
+static int launch_space(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int axis,
+                        int row0 = 0, int nrows = -1) {
     const Geom& G = c->G;
     SpaceParams P;
     P.src = src; P.dst = dst;
@@ -164,9 +166,12 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
     P.finf = s.f_inf; P.limiter = G.limiter;
     P.bc_lo = G.bc_lo; P.bc_hi = G.bc_hi;
     P.err = c->errflag;
+    P.row0 = axis == 0 ? row0 : 0;
+    if (nrows < 0) nrows = G.nyg;
+    if (nrows == 0) return VLASOV_OK;
     const int threads = 128;
     const long chunks = s.nvtot / 2;
-    dim3 grid((unsigned)((chunks + threads - 1) / threads), (unsigned)(axis == 0 ? G.nyg : G.nx));
+    dim3 grid((unsigned)((chunks + threads - 1) / threads), (unsigned)(axis == 0 ? nrows : G.nx));
     {
         Launch L(c, axis == 0 ? K_SWEEP_X : K_SWEEP_Y);
         sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
@@ -176,6 +181,9 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
 
 int launch_sweep_x(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts) {
     return launch_space(c, s, src, dst, dts, 0);
+}
+int launch_sweep_x_rows(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int row0, int nrows) {
+    return launch_space(c, s, src, dst, dts, 0, row0, nrows);
 }
 int launch_sweep_y(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts) {
     return launch_space(c, s, src, dst, dts, 1);

@@ -115,65 +115,6 @@ int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
 
-// ------------------------------------------------------------------------------------------------
-// Flux through face k (between cells k-1 and k, 1 <= k <= N-1) of a ZERO-PADDED line in shared memory:
-// L points at cell 0, stride st, and cells -3..-1 and N..N+2 hold zeros (f = 0 outside the velocity box,
-// R7), so the three reads around the foot cell need no bounds checks.  eq. (46) for sigma >= 0, eq. (47)
-// (sum repaired, R5) for sigma < 0: the same expression on the mirrored line.
-// ------------------------------------------------------------------------------------------------
-// ---- shared memory by 32-bit address (keeps the window base out of the inner loops) ----------------
-__device__ __forceinline__ double lds(unsigned a) {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
-    return v;
-}
-__device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v)); }
-__device__ __forceinline__ void cp_async8(unsigned dst, const double* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-
-// max(x, 0) on the bit pattern (no NaN fix-up code): x if its sign bit is clear, else +0.
-__device__ __forceinline__ double relu_bits(double x) {
-    const int h = __double2hiint(x);
-    const int m = ~(h >> 31);
-    return __hiloint2double(h & m, __double2loint(x) & m);
-}
-
-// Limited slopes eps+ d+, eps- d- of eqs. (43), (44) (R6) in the division-free clamp form
-//     eps+ d+ = clamp(d+, -max(0,Bv), max(0,A)),  eps- d- = clamp(d-, -max(0,A), max(0,Bv)),  A = 2 f0, Bv = 2 (f_inf - f0)
-// written in sign/magnitude: |eps d| = min(|d|, bound picked by the sign of d).  fp64 issue slots are the
-// scarce resource on this path, so the test "does any lane of the warp
-// need limiting at all" is done on the HIGH WORDS of the doubles in the integer pipe: for non-negative
-// doubles the IEEE order is the integer order, so
-//     hi(|d|) < min(hi(2 f0), hi(2 (f_inf - f0)))   ==>   |d| < min(2 f0, 2 (f_inf - f0))   ==>   eps = 1.
-// The test is conservative (ties and negative bounds fall through to the exact clamps); hi(2 x) is
-// hi(x) + 2^20 (exponent + 1; the denormal corner only ever errs by < 1e-307).
-template <int LIM>
-__device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, double finf, double& sp, double& sm) {
-    const double dp = fp - f0, dm = f0 - fm;
-    sp = dp; sm = dm;
-    if (LIM) {
-        const double g = finf - f0;
-        const int hb = min(__double2hiint(f0), __double2hiint(g)) + 0x00100000;
-        const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
-        const bool need = max(hp, hm) >= hb;
-        if (__any_sync(__activemask(), need)) {
-            const double hiA = relu_bits(f0 + f0), hiB = relu_bits(g + g);
-            const bool pneg = __double2hiint(dp) < 0, mneg = __double2hiint(dm) < 0;
-            const double bp = pneg ? hiB : hiA;
-            const double bm = mneg ? hiA : hiB;
-            const double ap = __hiloint2double(hp, __double2loint(dp));      // |d+|
-            const double am = __hiloint2double(hm, __double2loint(dm));      // |d-|
-            const double mp = ap < bp ? ap : bp;
-            const double mm = am < bm ? am : bm;
-            sp = __hiloint2double(__double2hiint(mp) | (__double2hiint(dp) & 0x80000000), __double2loint(mp));
-            sm = __hiloint2double(__double2hiint(mm) | (__double2hiint(dm) & 0x80000000), __double2loint(mm));
-        }
-    }
-}
-
 // Flux through face k (between cells k-1 and k, 1 <= k <= N-1) of a ZERO-PADDED line in shared memory:
 // L = shared byte address of cell 0, st8 = stride in bytes, cells -3..-1 and N..N+2 hold zeros (f = 0
 // outside the box, R7).  eq. (46) for sigma >= 0, eq. (47) (sum repaired, R5) for sigma < 0: the same

@@ -50,6 +50,7 @@ struct vlasov_ctx {
     double* fields_stage;// [6][nyg*nx] device staging of E,B for vlasov_step_host
     int* errflag;        // device int: first asynchronous error
     int mom_valid;
+    int fuse_xy;         // 1: use the fused spatial stage where it applies (vlasov_set_option)
     int64_t launches;
     int* h_err;          // pinned host mirror of errflag
     double* Jbuf;        // [3][nyg*nx] current density of vlasov_cycle
@@ -66,7 +67,7 @@ struct vlasov_ctx {
 namespace vl {
 
 enum Kind { K_SWEEP_X = 0, K_SWEEP_Y, K_TABLE, K_VSWEEP_X, K_VSWEEP_YZ, K_MOMENTS, K_GHOST_TABLE, K_CURRENT,
-            K_MAXWELL, K_COUNT };
+            K_MAXWELL, K_SWEEP_XY, K_COUNT };
 
 // Counts a launch and, when timing is on, brackets it with an event pair on the context's stream.
 struct Launch {
@@ -88,6 +89,11 @@ struct Launch {
 // spatial half sweeps, out of place src -> dst (a1, a2, a7, a8 of DESIGN.md)
 int launch_sweep_x(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);
 int launch_sweep_y(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);
+// x sweep of rows [row0, row0+nrows) only (ghost rows beside a fused stage)
+int launch_sweep_x_rows(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int row0, int nrows);
+// fused spatial stage (sweep_space_fused.cu): x then y (xfirst) or y then x, interior rows, src -> dst
+bool fused_xy_applicable(const vlasov_ctx* c, const Species& s, double dts);
+int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int xfirst);
 // Lorentz table (a3) and velocity sweeps (a4-a6), in place on f, rows [row0, row0+nrows)
 int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const double* B, double dt);
 int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows);
@@ -126,6 +132,59 @@ __device__ __forceinline__ double partial_flux(double fm, double f0, double fp, 
     double c1 = t * (2.0 - b);
     double c2 = t * (1.0 + b);
     return b * (f0 + c1 * sp + c2 * sm);
+}
+
+// ---- shared memory by 32-bit address (keeps the window base out of the inner loops) ----------------
+__device__ __forceinline__ double lds(unsigned a) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v)); }
+__device__ __forceinline__ void cp_async8(unsigned dst, const double* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+// max(x, 0) on the bit pattern (no NaN fix-up code): x if its sign bit is clear, else +0.
+__device__ __forceinline__ double relu_bits(double x) {
+    const int h = __double2hiint(x);
+    const int m = ~(h >> 31);
+    return __hiloint2double(h & m, __double2loint(x) & m);
+}
+
+// Limited slopes eps+ d+, eps- d- of eqs. (43), (44) (R6) in the division-free clamp form
+//     eps+ d+ = clamp(d+, -max(0,Bv), max(0,A)),  eps- d- = clamp(d-, -max(0,A), max(0,Bv)),  A = 2 f0, Bv = 2 (f_inf - f0)
+// written in sign/magnitude: |eps d| = min(|d|, bound picked by the sign of d).  fp64 issue slots are the
+// scarce resource on this path, so the test "does any lane of the warp
+// need limiting at all" is done on the HIGH WORDS of the doubles in the integer pipe: for non-negative
+// doubles the IEEE order is the integer order, so
+//     hi(|d|) < min(hi(2 f0), hi(2 (f_inf - f0)))   ==>   |d| < min(2 f0, 2 (f_inf - f0))   ==>   eps = 1.
+// The test is conservative (ties and negative bounds fall through to the exact clamps); hi(2 x) is
+// hi(x) + 2^20 (exponent + 1; the denormal corner only ever errs by < 1e-307).
+template <int LIM>
+__device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, double finf, double& sp, double& sm) {
+    const double dp = fp - f0, dm = f0 - fm;
+    sp = dp; sm = dm;
+    if (LIM) {
+        const double g = finf - f0;
+        const int hb = min(__double2hiint(f0), __double2hiint(g)) + 0x00100000;
+        const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
+        const bool need = max(hp, hm) >= hb;
+        if (__any_sync(__activemask(), need)) {
+            const double hiA = relu_bits(f0 + f0), hiB = relu_bits(g + g);
+            const bool pneg = __double2hiint(dp) < 0, mneg = __double2hiint(dm) < 0;
+            const double bp = pneg ? hiB : hiA;
+            const double bm = mneg ? hiA : hiB;
+            const double ap = __hiloint2double(hp, __double2loint(dp));      // |d+|
+            const double am = __hiloint2double(hm, __double2loint(dm));      // |d-|
+            const double mp = ap < bp ? ap : bp;
+            const double mm = am < bm ? am : bm;
+            sp = __hiloint2double(__double2hiint(mp) | (__double2hiint(dp) & 0x80000000), __double2loint(mp));
+            sm = __hiloint2double(__double2hiint(mm) | (__double2hiint(dm) & 0x80000000), __double2loint(mm));
+        }
+    }
 }
 
 // n = floor(s) for s >= 0 up to the exact-integer case, where n = s - 1, b = 1 is returned instead:

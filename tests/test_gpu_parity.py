@@ -62,11 +62,14 @@ def smooth_random_f(rng, w, s):
     return np.ascontiguousarray(f)
 
 
-def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None):
+def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None, fuse=None):
     """One vlasov_step on both sides.  Returns (f_gpu list, f_orc list, mom_gpu list, mom_orc list, code)."""
     import torch
     fg = [dev(f) for f in f0]
     ctx = gpu.context_for(w, fg, order=order, limiter=limiter)
+    if fuse is not None:
+        ctx.vlasov_set_option(gpu.OPT_FUSE_XY, fuse)
+    ctx.vlasov_timing_enable(True)
     keep = []
     if fluid is not None:
         for s in range(len(w.species)):
@@ -77,6 +80,8 @@ def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None):
     Ed, Bd = dev(E), dev(B)
     ctx.vlasov_step(dt, Ed, Bd, stages)
     code = ctx.check_code()
+    run_both.kinds = ctx.vlasov_timing_read()
+    ctx.vlasov_timing_enable(False)
     momg = []
     for s in range(len(w.species)):
         m = torch.empty((10, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
@@ -110,6 +115,31 @@ def test_spatial_half_steps(gpu, orc, bc, stages):
     assert rel_l2(fg[0], fo[0]) <= TOL1
     assert np.abs(fg[0] - fo[0]).max() <= 1e-13
     assert rel_l2(mg[0], mo[0]) <= TOL1
+
+
+@pytest.mark.parametrize("bc,g", [(inputs.BC_PERIODIC, 0), (inputs.BC_REFLECT, 0), (inputs.BC_FLUID, 2), (inputs.BC_FLUID, 3)])
+@pytest.mark.parametrize("nx,nv", [(13, (6, 8, 10)), (12, (4, 4, 8)), (16, (6, 8, 16)), (24, (3, 6, 32))])
+@pytest.mark.parametrize("stages", [1, 4])
+def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
+    """a1+a2 / a7+a8 as ONE fused pass (all |sigma| < 1): x blocks of 1, 4, 8 cells, chunks of 2..32 velocity cells
+    made of part of a v_z row / several rows, every y boundary kind; against the oracle and against the general
+    one-direction kernels."""
+    rng = np.random.default_rng(5)
+    w = random_workload(rng, nx=nx, ny=7, nv=nv, g=g, bc=bc)
+    f0 = [smooth_random_f(rng, w, 0)]
+    Z = np.zeros((3, w.ny_g, w.nx))
+    dt = 0.05          # |sigma_x| <= 4 * 0.025 / (1.7/24) = 0.71 ... 0.38; |sigma_y| <= 3 * 0.025 / (0.9/7) = 0.58
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, Z, Z, dt, stages, fuse=1)
+    assert code == 0
+    assert run_both.kinds["sweep_xy"][1] == 1 and run_both.kinds["sweep_y"][1] == 0      # the fused kernel ran
+    assert run_both.kinds["sweep_x"][1] == (2 if g else 0)                               # ghost rows: x sweep only
+    assert rel_l2(fg[0], fo[0]) <= TOL1
+    assert np.abs(fg[0] - fo[0]).max() <= 1e-13
+    assert rel_l2(mg[0], mo[0]) <= TOL1
+    fu, _, _, _, code = run_both(gpu, orc, w, f0, Z, Z, dt, stages, fuse=0)
+    assert code == 0
+    assert run_both.kinds["sweep_xy"][1] == 0 and run_both.kinds["sweep_y"][1] == 1
+    assert rel_l2(fg[0], fu[0]) <= TOL1
 
 
 @pytest.mark.parametrize("fields_yee", [0, 1])
