@@ -13,6 +13,9 @@
 //   * y is private to a thread: a 2-cell register window plus the previous flux per owned cell.
 // Rows -2, -1 and ny, ny+1 are the boundary rows of the y sweep (R16, R19): periodic wrap, the wall
 // image f(y_w + eta, vy) = f(y_w - eta, -vy), or FLUID ghost rows; they are loaded like any row.
+#include <cstdlib>
+#include <type_traits>
+#include <cuda.h>      // CUtensorMap (types only; the encoder is fetched through the runtime, no -lcuda)
 #include "vlasov_internal.cuh"
 
 namespace vl {
@@ -53,6 +56,12 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// 2D tiled TMA: box {PC cells, nx spatial cells} of row `c1 / nx` lands dense in shared memory as [x][PC]
+__device__ __forceinline__ void tma_g2s_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
 
 struct Weights {
@@ -130,7 +139,7 @@ __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH],
 // One step of the y march of an owned cell: rows (r-2, r-1, r) = (ya, yb, gx) -> new average h of row r-1
 // (sigma_y >= 0, eq. 46) or r-2 (sigma_y < 0, eq. 47 on the mirrored line).
 template <int LIM>
-__device__ __forceinline__ double y_step(double& ya, double& yb, double& yG, double gx, const Weights& Wy, double finf) {
+__device__ __forceinline__ double y_step(double ya, double yb, double& yG, double gx, const Weights& Wy, double finf) {
     const double dlo = yb - ya, dhi = gx - yb;
     double sp = Wy.pos ? dhi : -dlo, sm = Wy.pos ? dlo : -dhi;
     if (LIM) {
@@ -140,7 +149,7 @@ __device__ __forceinline__ double y_step(double& ya, double& yb, double& yG, dou
     }
     const double Gn = fma(Wy.w2, sm, fma(Wy.w1, sp, Wy.w0 * yb));
     const double h = Wy.pos ? yb + (yG - Gn) : ya + (Gn - yG);
-    yG = Gn; ya = yb; yb = gx;
+    yG = Gn;
     return h;
 }
 
@@ -159,9 +168,12 @@ __device__ __forceinline__ int virtual_row(const XYParams& P, int r, bool& mirro
 
 // XFIRST = 1: x remap of every incoming row, then the y march (a1 + a2).
 // XFIRST = 0: y march on the raw rows, then the x remap of every finished row (a7 + a8).
-// Shared memory: [2 mbarriers][raw row 0][raw row 1]([y-swept row 0][y-swept row 1] if !XFIRST).
+// Shared memory: [NS mbarriers][NS raw rows]([2 y-swept rows] if !XFIRST).  Raw rows arrive by bulk TMA, NS - 1
+// rows ahead of the row being worked on.
+constexpr int XY_NS = 3;
+
 template <int XB, int LIM, int XFIRST>
-__global__ void __launch_bounds__(512, 1) sweep_xy_kernel(XYParams P) {
+__global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant__ CUtensorMap tmap, XYParams P) {
     extern __shared__ __align__(128) unsigned char smraw[];
     const int C = P.C, C8 = C * 8;
     const int c = threadIdx.x % C, blk = threadIdx.x / C;
@@ -170,126 +182,203 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(XYParams P) {
     const long v = v0 + c;
     const int ivx = (int)(v / ((long)P.nv1 * P.nv2));
     const int ivy = (int)((v / P.nv2) % P.nv1);
-    Weights Wx, Wy;
-    Wx.set((P.vminx + (ivx + 0.5) * P.dvx) * P.kx);
-    Wy.set((P.vminy + (ivy + 0.5) * P.dvy) * P.ky);
+    // the six weights of a velocity cell live in shared memory (wt[k][c]): 12 registers less per thread; only
+    // the two flow directions stay in registers
+    double* wt = reinterpret_cast<double*>(smraw + 128);
+    bool xpos, ypos;
+    {
+        Weights W0x, W0y;
+        W0x.set((P.vminx + (ivx + 0.5) * P.dvx) * P.kx);
+        W0y.set((P.vminy + (ivy + 0.5) * P.dvy) * P.ky);
+        xpos = W0x.pos; ypos = W0y.pos;
+        if (blk == 0) {
+            wt[0 * C + c] = W0x.w0; wt[1 * C + c] = W0x.w1; wt[2 * C + c] = W0x.w2;
+            wt[3 * C + c] = W0y.w0; wt[4 * C + c] = W0y.w1; wt[5 * C + c] = W0y.w2;
+        }
+    }
     const unsigned bar0 = smem_addr(smraw);
-    const unsigned rowbytes = (unsigned)P.nx * C8;
-    const unsigned raw0 = bar0 + 128;
-    const unsigned hb0 = raw0 + 2 * rowbytes;
-    const unsigned cofs = c * 8;
-    const unsigned own = (unsigned)ix0 * C8 + cofs;
+    // a row buffer is made of C / PC pieces, each a dense [x][PC] TMA box (128-byte aligned)
+    const int PC = P.PC, npp = C / PC, X8 = PC * 8;
+    const unsigned piecebytes = ((unsigned)P.nx * X8 + 127u) & ~127u;
+    const unsigned rowbytes = piecebytes * npp;
+    const unsigned raw0 = bar0 + 128 + ((6 * C * 8 + 127) & ~127);
+    const unsigned hb0 = raw0 + XY_NS * rowbytes;
+    const unsigned cofs = (unsigned)(c / PC) * piecebytes + (unsigned)(c % PC) * 8;
+    const unsigned own = (unsigned)ix0 * X8 + cofs;
     const double finf = P.finf;
 
-    // producer side: piece t of a row = PC contiguous cells of one x (a v_z row or a part of one, so that its
-    // wall image is contiguous too); the pieces are spread over the threads
-    const int PC = P.PC, npp = C / PC;               // pieces per x
-    const int ncopy = P.nx * npp;
-    auto issue_row = [&](int r) {
-        const unsigned bar = bar0 + 8 * (r & 1);
-        if (threadIdx.x == 0) mbar_expect_tx(bar, rowbytes);
-        bool m; const int ar = virtual_row(P, r, m);
-        for (int t = threadIdx.x; t < ncopy; t += blockDim.x) {
-            const int cp_ix = t / npp, cp_pc = t - cp_ix * npp;
-            const long vp = v0 + (long)cp_pc * PC;
-            long src = (long)ar * P.row_stride + (long)cp_ix * P.S + vp;
-            if (m) src += (long)(P.nv1 - 1 - 2 * (int)((vp / P.nv2) % P.nv1)) * P.nv2;     // i_vy mirrored (R19)
-            bulk_g2s(raw0 + (r & 1) * rowbytes + (unsigned)(cp_ix * C + cp_pc * PC) * 8, P.src + src, (unsigned)PC * 8, bar);
+    // producer: thread 0 issues one tiled TMA load per piece and row (a piece = PC contiguous cells of every x:
+    // a v_z row or a part of one, so that its wall image, i_vy mirrored (R19), is one box too)
+    auto issue_row = [&](int r, int stage) {
+        if (threadIdx.x == 0) {
+            const unsigned bar = bar0 + 8 * stage;
+            mbar_expect_tx(bar, (unsigned)P.nx * C8);
+            bool m; const int ar = virtual_row(P, r, m);
+            for (int p = 0; p < npp; ++p) {
+                long vp = v0 + (long)p * PC;
+                if (m) vp += (long)(P.nv1 - 1 - 2 * (int)((vp / P.nv2) % P.nv1)) * P.nv2;
+                tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes, &tmap, (int)vp, ar * P.nx, bar);
+            }
         }
     };
-    if (threadIdx.x == 0) { mbar_init(bar0, 1); mbar_init(bar0 + 8, 1); }
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < XY_NS; ++i) mbar_init(bar0 + 8 * i, 1);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
-    // thread 0 arms the barrier before any copy of that row can complete: the arming and the copies of a
-    // row are issued after the same __syncthreads, thread 0's expect_tx first within its warp
-    issue_row(-2);
-    issue_row(-1);
+    // a barrier's phase cannot complete before thread 0's arrive.expect_tx, whatever order the copies land in
+    const int rlast = P.ny + 1;
+    for (int i = 0; i < XY_NS - 1; ++i) if (-2 + i <= rlast) issue_row(-2 + i, i);
 
-    double ya[XB], yb[XB], yG[XB];
+    // y window of the owned cells: rows r-2 and r-1 sit in A and B, swapping roles every row (no moves)
+    double A[XB], B[XB], yG[XB];
 #pragma unroll
-    for (int i = 0; i < XB; ++i) { ya[i] = 0.0; yb[i] = 0.0; yG[i] = 0.0; }
-    const int orow_shift = Wy.pos ? 1 : 2;
-    for (int r = -2; r <= P.ny + 1; ++r) {
-        const int st = r & 1;
-        const unsigned sraw = raw0 + st * rowbytes;
-        mbar_wait(bar0 + 8 * st, ((r + 2) >> 1) & 1);
+    for (int i = 0; i < XB; ++i) { A[i] = 0.0; B[i] = 0.0; yG[i] = 0.0; }
+    const int orow_shift = ypos ? 1 : 2;
+    constexpr int CH = XB < 4 ? XB : 4;
+
+    // one row; PAR = parity of r + 2: rows (r-2, r-1) = (A, B) if PAR == 0 else (B, A); the new row replaces r-2
+    auto row = [&](auto par, int r, int stage, unsigned phase) {
+        constexpr int PAR = decltype(par)::value;
+        Weights Wx, Wy;
+        Wx.w0 = wt[0 * C + c]; Wx.w1 = wt[1 * C + c]; Wx.w2 = wt[2 * C + c]; Wx.pos = xpos;
+        Wy.w0 = wt[3 * C + c]; Wy.w1 = wt[4 * C + c]; Wy.w2 = wt[5 * C + c]; Wy.pos = ypos;
+        const unsigned sraw = raw0 + stage * rowbytes;
+        mbar_wait(bar0 + 8 * stage, phase);
         const int orow = r - orow_shift;
         double* po = P.dst + (long)(P.g + orow) * P.row_stride + (long)ix0 * P.S + v;
         const bool store = orow >= 0 && orow < P.ny;
-        constexpr int CH = XB < 4 ? XB : 4;
+        const int nstage = stage == 0 ? XY_NS - 1 : stage - 1;      // stage of row r + NS - 1 = stage of row r - 1
         if (XFIRST) {
+            // row r - 1 was left by every thread before the __syncthreads that ended it: refill its stage
+            if (r + XY_NS - 1 <= rlast) issue_row(r + XY_NS - 1, nstage);
             double carry = 0.0;
 #pragma unroll
             for (int k = 0; k < XB / CH; ++k) {
                 double gx[CH];
-                if (Wx.pos) x_chunk<XB, CH, LIM, 1>(k, carry, gx, sraw, ix0, P.nx, C8, cofs, Wx, finf);
-                else        x_chunk<XB, CH, LIM, -1>(k, carry, gx, sraw, ix0, P.nx, C8, cofs, Wx, finf);
+                if (Wx.pos) {
+                    x_chunk<XB, CH, LIM, 1>(k, carry, gx, sraw, ix0, P.nx, X8, cofs, Wx, finf);
 #pragma unroll
-                for (int i = 0; i < CH; ++i) {
-                    // the item index is a compile-time constant on either branch
-                    if (Wx.pos) {
-                        constexpr int dummy = 0; (void)dummy;
+                    for (int i = 0; i < CH; ++i) {
                         const int it = k * CH + i;
-                        const double h = y_step<LIM>(ya[it], yb[it], yG[it], gx[i], Wy, finf);
+                        const double h = PAR == 0 ? y_step<LIM>(A[it], B[it], yG[it], gx[i], Wy, finf)
+                                                  : y_step<LIM>(B[it], A[it], yG[it], gx[i], Wy, finf);
+                        if (PAR == 0) A[it] = gx[i]; else B[it] = gx[i];
                         if (store) __stcs(po + (long)it * P.S, h);
-                    } else {
+                    }
+                } else {
+                    x_chunk<XB, CH, LIM, -1>(k, carry, gx, sraw, ix0, P.nx, X8, cofs, Wx, finf);
+#pragma unroll
+                    for (int i = 0; i < CH; ++i) {
                         const int it = XB - 1 - (k * CH + i);
-                        const double h = y_step<LIM>(ya[it], yb[it], yG[it], gx[i], Wy, finf);
+                        const double h = PAR == 0 ? y_step<LIM>(A[it], B[it], yG[it], gx[i], Wy, finf)
+                                                  : y_step<LIM>(B[it], A[it], yG[it], gx[i], Wy, finf);
+                        if (PAR == 0) A[it] = gx[i]; else B[it] = gx[i];
                         if (store) __stcs(po + (long)it * P.S, h);
                     }
                 }
             }
             __syncthreads();                       // everybody is done reading raw row r
-            if (r + 2 <= P.ny + 1) issue_row(r + 2);
         } else {
-            const unsigned sh = hb0 + st * rowbytes;
+            const unsigned sh = hb0 + (unsigned)PAR * rowbytes;
 #pragma unroll
             for (int i = 0; i < XB; ++i) {
-                const double h = y_step<LIM>(ya[i], yb[i], yG[i], lds(sraw + own + i * C8), Wy, finf);
-                sts(sh + own + i * C8, h);
+                const double gx = lds(sraw + own + i * X8);
+                const double h = PAR == 0 ? y_step<LIM>(A[i], B[i], yG[i], gx, Wy, finf)
+                                          : y_step<LIM>(B[i], A[i], yG[i], gx, Wy, finf);
+                if (PAR == 0) A[i] = gx; else B[i] = gx;
+                sts(sh + own + i * X8, h);
             }
-            __syncthreads();                       // y-swept row complete; raw row r free
-            if (r + 2 <= P.ny + 1) issue_row(r + 2);
+            __syncthreads();                       // y-swept row complete; raw rows up to r are free
+            if (r + XY_NS <= rlast) issue_row(r + XY_NS, stage);
             double carry = 0.0;
 #pragma unroll
             for (int k = 0; k < XB / CH; ++k) {
                 double o[CH];
-                if (Wx.pos) x_chunk<XB, CH, LIM, 1>(k, carry, o, sh, ix0, P.nx, C8, cofs, Wx, finf);
-                else        x_chunk<XB, CH, LIM, -1>(k, carry, o, sh, ix0, P.nx, C8, cofs, Wx, finf);
-                if (store) {
+                if (Wx.pos) {
+                    x_chunk<XB, CH, LIM, 1>(k, carry, o, sh, ix0, P.nx, X8, cofs, Wx, finf);
+                    if (store) {
 #pragma unroll
-                    for (int i = 0; i < CH; ++i) {
-                        const int it = Wx.pos ? k * CH + i : XB - 1 - (k * CH + i);
-                        __stcs(po + (long)it * P.S, o[i]);
+                        for (int i = 0; i < CH; ++i) __stcs(po + (long)(k * CH + i) * P.S, o[i]);
+                    }
+                } else {
+                    x_chunk<XB, CH, LIM, -1>(k, carry, o, sh, ix0, P.nx, X8, cofs, Wx, finf);
+                    if (store) {
+#pragma unroll
+                        for (int i = 0; i < CH; ++i) __stcs(po + (long)(XB - 1 - (k * CH + i)) * P.S, o[i]);
                     }
                 }
             }
+        }
+    };
+    if (!XFIRST) { if (XY_NS - 3 <= rlast) issue_row(-2 + XY_NS - 1, XY_NS - 1); }   // !XFIRST refills after its barrier: start one row deeper
+    int stage = 0; unsigned phase = 0;
+    for (int r = -2; r <= rlast; r += 2) {
+        row(std::integral_constant<int, 0>{}, r, stage, phase);
+        if (++stage == XY_NS) { stage = 0; phase ^= 1; }
+        if (r + 1 <= rlast) {
+            row(std::integral_constant<int, 1>{}, r + 1, stage, phase);
+            if (++stage == XY_NS) { stage = 0; phase ^= 1; }
         }
     }
 }
 
 template <int XB, int LIM>
-static void launch_xy_t(const XYParams& P, int xfirst, dim3 grid, int threads, size_t smem, cudaStream_t st) {
+static void launch_xy_t(const CUtensorMap& tm, const XYParams& P, int xfirst, dim3 grid, int threads, size_t smem,
+                        cudaStream_t st) {
     if (xfirst) {
         cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        sweep_xy_kernel<XB, LIM, 1><<<grid, threads, smem, st>>>(P);
+        sweep_xy_kernel<XB, LIM, 1><<<grid, threads, smem, st>>>(tm, P);
     } else {
         cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        sweep_xy_kernel<XB, LIM, 0><<<grid, threads, smem, st>>>(P);
+        sweep_xy_kernel<XB, LIM, 0><<<grid, threads, smem, st>>>(tm, P);
     }
+}
+
+// Tensor map of one species' f seen as a matrix [ny_g * nx spatial cells][S velocity cells] of fp64, box
+// {pc cells, nx spatial cells}.  The encoder is a driver entry point fetched through the runtime.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static bool make_row_map(CUtensorMap* tm, const double* base, long S, long ncell, int pc, int nx) {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || !p) return false;
+        fn = (EncodeTiledFn)p;
+    }
+    const cuuint64_t dims[2] = {(cuuint64_t)S, (cuuint64_t)ncell};
+    const cuuint64_t strides[1] = {(cuuint64_t)S * 8};
+    const cuuint32_t box[2] = {(cuuint32_t)pc, (cuuint32_t)nx};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Shared memory of the fused kernel: barriers, weight table, NS raw rows (+ 2 y-swept rows), each row made of
+// 128-byte aligned pieces.
+static size_t xy_smem_bytes(const Geom& G, const Species& s, int C, int xfirst) {
+    const int pc = C < s.nv[2] ? C : s.nv[2];
+    const size_t piece = ((size_t)G.nx * pc * 8 + 127) & ~(size_t)127;
+    const size_t row = piece * (C / pc);
+    return 128 + ((6 * (size_t)C * 8 + 127) & ~(size_t)127) + (xfirst ? XY_NS : XY_NS + 2) * row;
 }
 
 // Tile shape of the fused stage: XB x cells per thread, C contiguous velocity cells per CTA -- a power of two
 // that divides the block, made of whole v_z rows or a part of one, at least 16 bytes, at most 512 threads.
 static bool pick_xy_shape(const Geom& G, const Species& s, int& xb, int& C) {
     xb = 1;
-    if (G.nx % 8 == 0) xb = 8; else if (G.nx % 4 == 0) xb = 4;
+    // 4 x cells per thread: 8 would halve the halo work but spills at the 128-register cap of 512 threads
+    static const char* force = getenv("VLASOV_XB");        // tuning aid: VLASOV_XB=8
+    if (G.nx % 8 == 0 && force && force[0] == '8') xb = 8; else if (G.nx % 4 == 0) xb = 4;
     const int nblk = G.nx / xb;
     C = 32;
     auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && nblk * cc <= 512; };
     while (C >= 2 && !ok(C)) C >>= 1;
     if (C < 2) return false;
-    return 128 + 4 * (size_t)G.nx * C * 8 <= 200 * 1024;
+    if (G.nx > 256) return false;                  // TMA box limit
+    return xy_smem_bytes(G, s, C, 0) <= 200 * 1024;
 }
 
 // Whether the fused stage applies: all shifts below one cell, at least two cells per direction, two ghost
@@ -327,15 +416,17 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     const int nblk = G.nx / xb;
     P.C = C;
     P.PC = C < s.nv[2] ? C : s.nv[2];
-    const size_t smem = 128 + (xfirst ? 2 : 4) * (size_t)G.nx * C * 8;
+    const size_t smem = xy_smem_bytes(G, s, C, xfirst);
+    CUtensorMap tm;
+    if (!make_row_map(&tm, src, s.nvtot, (long)G.nyg * G.nx, P.PC, G.nx)) return VLASOV_ECUDA;
     dim3 grid((unsigned)(s.nvtot / C));
     const int threads = nblk * C;
     const int lim = G.limiter ? 1 : 0;
     {
         Launch L(c, K_SWEEP_XY);
-        if (xb == 8) { if (lim) launch_xy_t<8, 1>(P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<8, 0>(P, xfirst, grid, threads, smem, c->stream); }
-        else if (xb == 4) { if (lim) launch_xy_t<4, 1>(P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0>(P, xfirst, grid, threads, smem, c->stream); }
-        else { if (lim) launch_xy_t<1, 1>(P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0>(P, xfirst, grid, threads, smem, c->stream); }
+        if (xb == 8) { if (lim) launch_xy_t<8, 1>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<8, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (xb == 4) { if (lim) launch_xy_t<4, 1>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else { if (lim) launch_xy_t<1, 1>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
     }
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
