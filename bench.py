@@ -186,6 +186,24 @@ def oracle_leg(w, steps, warmup, budget_s=25.0):
 
 
 # ------------------------------------------------------------------------------------------------
+# multi-GPU: replicas only -- the only cross-rank step is the timing reduction
+# ------------------------------------------------------------------------------------------------
+def max_over_ranks(ms, dist, device):
+    """Device-timed milliseconds -> the maximum over all ranks (identity without a process group)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cells_per_replica, steps, ms, world):
+    """Aggregate cell-updates/s of `world` independent replicas that all ran `steps` steps within `ms`."""
+    return world * cells_per_replica * steps / (ms * 1e-3)
+
+
+# ------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------
 def upload_f(w, s, torch, device):
@@ -269,12 +287,9 @@ def gpu_arm(args):
     ms = ev0.elapsed_time(ev1)
     per_kind = ctx.vlasov_timing_read()
     ctx.vlasov_timing_enable(False)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, device)
     cells = w.interior_cells
-    value = world * cells * args.steps / (ms * 1e-3)
+    value = whole_job_value(cells, args.steps, ms, world)
 
     # ---- end-to-end leg: HOST buffers through the C ABI (vlasov_cycle_host) -----------------
     ncell = w.ny_g * w.nx
@@ -293,11 +308,8 @@ def gpu_arm(args):
     ev1.record(stream)
     barrier()
     ms_e = ev0.elapsed_time(ev1)
-    if dist is not None:
-        t = torch.tensor([ms_e], dtype=torch.float64, device=device)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e = float(t.item())
-    e2e = world * cells * e2e_steps / (ms_e * 1e-3)
+    ms_e = max_over_ranks(ms_e, dist, device)
+    e2e = whole_job_value(cells, e2e_steps, ms_e, world)
     h2d = 6 * ncell * 8
     d2h = (6 + 10 * ns) * ncell * 8
     if not np.isfinite(Mh.numpy()).all():
@@ -382,7 +394,7 @@ def reference_arm(args):
     if rank != 0:
         return
     w = make_workload(args.workload)
-    v, ms, cores, sample, done = oracle_leg(w, steps=args.steps, warmup=args.warmup, budget_s=150.0)
+    v, ms, cores, sample, done = oracle_leg(w, steps=args.steps, warmup=args.warmup, budget_s=args.ref_budget)
     out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise)",
@@ -401,7 +413,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="gem128")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle time for the cpu_baseline leg")
+    ap.add_argument("--ref-budget", type=float, default=150.0, help="seconds of oracle time for --impl reference")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

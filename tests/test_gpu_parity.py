@@ -367,3 +367,55 @@ def test_error_paths(gpu, orc):
     assert e.value.code == gpu.EALIGN
     cfg2 = gpu.make_config(0, 4, 0, 1, 1.0, 1.0, 0, 0)
     assert gpu.vlasov_scratch_bytes(cfg2, sp) == 0
+
+
+def test_full_size_gem128_sampled_window(gpu, orc):
+    """Config 3 at full size (128x64x32^3 x 2 species, 4.3 GB of f) in the launch configuration bench.py times: one
+    complete step on the GPU, then (i) properties that hold at any size -- relative mass drift <= 1e-13, f >= 0 --
+    and (ii) sampled parity: a 16x16 spatial window of the same inputs is advanced by the oracle; the domain of
+    dependence of one step is 4 cells per direction (two half sweeps, |sigma| < 1, stencil of 2), so the inner 6x6
+    cells of the window must agree with the full run whatever the window's own boundary."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 9 * 2**30:
+        pytest.skip("needs 9 GB of device memory")
+    w = inputs.gem_workload(nx=128, ny=64, nv=32, steps=1)
+    ix0, iy0, nw, margin = 40, 24, 16, 5
+    E, B = inputs.gem_fields(w)
+    fg, f0win, mass0 = [], [], []
+    for s, sp in enumerate(w.species):
+        sp.f_inf = inputs.gem_f_inf(w, s)
+        f = torch.empty((w.ny_g, w.nx) + tuple(sp.nv), dtype=torch.float64, device="cuda")
+        win = np.empty((nw, nw) + tuple(sp.nv))
+        for r in range(w.ny_g):
+            row = inputs.gem_f(w, s, rows=[r])[0]
+            f[r].copy_(torch.from_numpy(row))
+            if iy0 <= r < iy0 + nw:
+                win[r - iy0] = row[ix0:ix0 + nw]
+        fg.append(f)
+        f0win.append(win)
+        mass0.append(float(f.sum().item()))
+    ctx = gpu.context_for(w, fg)
+    ctx.vlasov_timing_enable(True)
+    Ed, Bd = dev(E), dev(B)
+    ctx.vlasov_step(w.dt, Ed, Bd, gpu.STAGE_ALL)
+    assert ctx.check_code() == 0
+    kinds = ctx.vlasov_timing_read()
+    assert kinds["sweep_xy"][1] == 4 and kinds["vsweep_yz"][1] == 2        # the configuration bench.py times
+    Ew = np.ascontiguousarray(E[:, iy0:iy0 + nw, ix0:ix0 + nw])
+    Bw = np.ascontiguousarray(B[:, iy0:iy0 + nw, ix0:ix0 + nw])
+    inner = slice(margin, nw - margin)
+    for s, sp in enumerate(w.species):
+        drift = abs(float(fg[s].sum().item()) - mass0[s]) / mass0[s]
+        assert drift <= 1e-13, (s, drift)
+        assert float(fg[s].min().item()) >= 0.0
+        fo = f0win[s].copy()
+        err, _ = orc.step(fo, osp(orc, sp), nw, nw, 0, nw * w.dx, nw * w.dy, w.dt, Ew, Bw, fields_yee=w.fields_yee,
+                          bc_lo=inputs.BC_PERIODIC, bc_hi=inputs.BC_PERIODIC, want_moments=False)
+        assert err == 0
+        got = fg[s][iy0:iy0 + nw, ix0:ix0 + nw].cpu().numpy()
+        assert rel_l2(got[inner, inner], fo[inner, inner]) <= TOL1, s
+        assert np.abs(got[inner, inner] - fo[inner, inner]).max() <= 1e-13 * sp.f_inf
+        # and the window's own edge does differ (the comparison is not vacuous)
+        assert rel_l2(got[0], fo[0]) > 1e-9
+    ctx.close()
