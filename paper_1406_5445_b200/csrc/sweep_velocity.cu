@@ -154,12 +154,82 @@ __device__ __forceinline__ double face_flux_pad(unsigned L, int st8, int N, int 
     return __hiloint2double(__double2hiint(phi) ^ (sg & 0x80000000), __double2loint(phi));
 }
 
+struct OutShared {       // cells of a line in shared memory: cell0 = byte address of cell a
+    unsigned a; int st8;
+    __device__ __forceinline__ void put(double v) { sts(a, v); a += st8; }
+    __device__ __forceinline__ void step(int dir) { st8 *= dir; }
+    __device__ __forceinline__ void skip(int n) { a += n * st8; }
+};
+struct OutGlobal {       // cells of a line in global memory (streaming store)
+    double* p; long st;
+    __device__ __forceinline__ void put(double v) { __stcs(p, v); p += st; }
+    __device__ __forceinline__ void step(int dir) { st *= dir; }
+    __device__ __forceinline__ void skip(int n) { p += n * st; }
+};
+
+// Does the slope pair (dp, dm) of a cell with value f0 possibly need limiting?  High-word test of slopes_fast
+// (conservative).  The sign bit of the result is set if so.
+__device__ __forceinline__ int need_bits(double f0, double dp, double dm, double finf) {
+    const int hb = min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000;
+    const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
+    return (hb - 1) - max(hp, hm);
+}
+
+// Segment of SEG cells [a, a+SEG) whose SEG+1 faces all have |sigma| < 1 (no whole cells in eqs. 46/47) and one
+// flow direction: the SEG+3 cells the fluxes touch are read ONCE into registers, in the direction of the flow
+// (eq. 47 = eq. 46 on the mirrored line), and face m of the walk takes (q[m], q[m+1], q[m+2]).  About a
+// quarter of the instructions of the general walk below.
+//   walk position i <-> cell a-2+i (sigma >= 0) | a+SEG+1-i (sigma < 0);  face m <-> face a+m | a+SEG-m.
+template <int SEG, int LIM, class Out>
+__device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
+                                                double s1, double finf, Out out) {
+    const bool pos = !(sig_a < 0.0 || sig_b < 0.0);      // the caller made sure the two do not disagree
+    const int dir = pos ? 1 : -1;
+    const int ust8 = pos ? st8 : -st8;
+    unsigned addr = L + (pos ? a - 2 : a + SEG + 1) * st8;
+    double q[SEG + 3];
+#pragma unroll
+    for (int i = 0; i < SEG + 3; ++i) { q[i] = lds(addr); addr += ust8; }
+    // box faces carry no flux (R7): the first / last face of the walk may be one
+    const bool zero_first = pos ? a == 0 : a + SEG == N;
+    const bool zero_last = pos ? a + SEG == N : a == 0;
+    double sig = pos ? sig_a : sig_b;
+    const double ds = pos ? s1 : -s1;
+    if (!pos) { out.skip(SEG - 1); }
+    out.step(dir);
+    double Gp = 0.0;
+#pragma unroll
+    for (int m = 0; m <= SEG; ++m) {
+        double sp, sm;
+        slopes_fast<LIM>(q[m], q[m + 1], q[m + 2], finf, sp, sm);     // all lanes sit on the same face: one vote per face
+        const double bq = fabs(sig);
+        const double b2 = bq * bq;
+        const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
+        const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+        double G = bq * fma(c1, sp, fma(c2, sm, q[m + 1]));
+        if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
+        if (m > 0) out.put(q[m + 1] + (Gp - G));     // eq. (38) for the cell between walk faces m-1 and m
+        Gp = G;
+        sig += ds;
+    }
+}
+
 // One thread remaps cells [a, b) of one line: flux per face, eq. (38) per cell.  sigma of face k is
 // s0 + s1 k (accumulated).  out.put(value) stores the new average of the next cell (a, a+1, ...).
-template <int LIM, class Out>
+template <int LIM, int FAST, class Out>
 __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
                                             double finf, Out& out) {
     double sig = fma(s1, (double)a, s0);
+    constexpr int SEG = 8;
+    if (FAST && b - a == SEG) {
+        // sigma is affine along the line: |sigma| < 1 and one sign at both end faces holds on every face between
+        const double sig_b = fma(s1, (double)b, s0);
+        const bool small = fabs(sig) < 1.0 && fabs(sig_b) < 1.0 && !(sig * sig_b < 0.0);
+        if (__all_sync(__activemask(), small)) {
+            march_seg_small<SEG, LIM>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            return;
+        }
+    }
     double phi_lo = a > 0 ? face_flux_pad<LIM>(L, st8, N, a, sig, finf) : 0.0;
     unsigned ci = L + a * st8;
     const int bi = b < N ? b : N - 1;                // faces a+1 .. bi are interior
@@ -173,15 +243,6 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
     }
     if (b == N) out.put(lds(ci) + phi_lo);           // zero flux through the upper box face (R7)
 }
-
-struct OutShared {       // consecutive cells of a line in shared memory
-    unsigned a; int st8;
-    __device__ __forceinline__ void put(double v) { sts(a, v); a += st8; }
-};
-struct OutGlobal {       // consecutive cells of a line in global memory (streaming store)
-    double* p; long st;
-    __device__ __forceinline__ void put(double v) { __stcs(p, v); p += st; }
-};
 
 // q = e / d, r = e % d with m = floor((2^32 - 1) / d): the estimate is at most 2 short.
 __device__ __forceinline__ void fast_divmod(unsigned e, unsigned d, unsigned m, unsigned& q, unsigned& r) {
@@ -212,7 +273,7 @@ constexpr int V_THREADS = 256;
 // Persistent: a CTA loops over tiles, the pad rows are zeroed once.
 // ------------------------------------------------------------------------------------------------
 template <int LIM>
-__global__ void __launch_bounds__(V_THREADS) vsweep_x_kernel(VParams P) {
+__global__ void __launch_bounds__(V_THREADS, 4) vsweep_x_kernel(VParams P) {
     extern __shared__ double sm[];
     const int CT = P.ct, N = P.nv0, H = CT >> 1;
     const int plane = P.nv1 * P.nv2;
@@ -242,7 +303,7 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_x_kernel(VParams P) {
                 const double s0 = t0 + t2 * k1 + t3 * k2;
                 const int a = seg * seglen, b = min(a + seglen, N);
                 OutGlobal o{fb + c + (long)a * plane, (long)plane};
-                march_cells<LIM>(smem_addr(A + c), CT * 8, N, a, b, s0, t1, finf, o);
+                march_cells<LIM, 0>(smem_addr(A + c), CT * 8, N, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
@@ -255,13 +316,19 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_x_kernel(VParams P) {
 // lines hit distinct banks), PS = (N1 + 3) RS, OFF = 3 RS + 3; everything that is not a cell is zero and
 // serves as the padding of the lines in both directions.  vy: A -> Bf; vz: Bf -> A; A -> global.
 // ------------------------------------------------------------------------------------------------
-template <int LIM>
-__global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
+// CN > 0: the velocity plane is CN x CN cells and the tile shape is the launcher's choice for it, all known at
+// compile time (strides become immediates, the staging loops unroll); CN = 0: any shape, at run time.
+template <int LIM, int CN>
+__global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
     extern __shared__ double sm[];
-    const int N1 = P.nv1, N2 = P.nv2;
+    const int N1 = CN ? CN : P.nv1, N2 = CN ? CN : P.nv2;
+    constexpr int CCT = CN ? (8 * V_THREADS) / (CN * CN) : 0;      // planes per tile, as launch_vsweeps picks them
+    constexpr int CSEG = CN ? (CN + 7) / 8 : 0;
+    if (CN && (P.ct != CCT || P.nseg != CSEG || P.nseg2 != CSEG)) return;
+    const int ct = CN ? CCT : P.ct, nseg1 = CN ? CSEG : P.nseg, nseg2 = CN ? CSEG : P.nseg2;
     const int plane = N1 * N2;
     const int RS = N2 + 3, PS = (N1 + 3) * RS, OFF = 3 * RS + 3;
-    const int BUF = (OFF + P.ct * PS + 1) & ~1;
+    const int BUF = (OFF + ct * PS + 1) & ~1;
     double* A = sm;
     double* Bf = sm + BUF;
     for (int e = threadIdx.x; e < 2 * BUF; e += V_THREADS) sm[e] = 0.0;
@@ -276,8 +343,8 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
     const unsigned dso = dz + dy * RS + (drow / N1) * PS;
     for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x) {
         const int cell = P.cell0 + tile / P.ntile;
-        const int p0 = (tile % P.ntile) * P.ct;
-        const int np = min(P.ct, P.nv0 - p0);
+        const int p0 = (tile % P.ntile) * ct;
+        const int np = ct;                          // equal tiles: ct divides nv0 (launch_vsweeps)
         double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
         const double* T = P.table + (long)cell * TAB;
         const int ncellt = np * plane;
@@ -295,29 +362,29 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
         __syncthreads();
         {   // vy: line along i_vy (stride RS); transverse (i_vx, i_vz); thread index runs along z
             const double t0 = T[4], t1 = T[5], t2 = T[6], t3 = T[7], finf = T[13];
-            const int seglen = (N1 + P.nseg - 1) / P.nseg;
+            const int seglen = (N1 + nseg1 - 1) / nseg1;
             const int nl = np * N2;
-            for (int wi = threadIdx.x; wi < nl * P.nseg; wi += V_THREADS) {
+            for (int wi = threadIdx.x; wi < nl * nseg1; wi += V_THREADS) {
                 const int seg = wi / nl, l = wi - seg * nl;
                 const int p = l / N2, z = l - p * N2;
                 const double s0 = t0 + t2 * (p0 + p) + t3 * z;
                 const int a = seg * seglen, b = min(a + seglen, N1);
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM>(smem_addr(A + OFF + p * PS + z), RS * 8, N1, a, b, s0, t1, finf, o);
+                march_cells<LIM, 1>(smem_addr(A + OFF + p * PS + z), RS * 8, N1, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
         {   // vz: contiguous lines; transverse (i_vx, i_vy); thread index runs along y (stride RS, odd)
             const double t0 = T[8], t1 = T[9], t2 = T[10], t3 = T[11], finf = T[14];
-            const int seglen = (N2 + P.nseg2 - 1) / P.nseg2;
+            const int seglen = (N2 + nseg2 - 1) / nseg2;
             const int nl = np * N1;
-            for (int wi = threadIdx.x; wi < nl * P.nseg2; wi += V_THREADS) {
+            for (int wi = threadIdx.x; wi < nl * nseg2; wi += V_THREADS) {
                 const int seg = wi / nl, l = wi - seg * nl;
                 const int p = l / N1, y = l - p * N1;
                 const double s0 = t0 + t2 * (p0 + p) + t3 * y;
                 const int a = seg * seglen, b = min(a + seglen, N2);
                 OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
-                march_cells<LIM>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, t1, finf, o);
+                march_cells<LIM, 1>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
@@ -335,8 +402,8 @@ __global__ void __launch_bounds__(V_THREADS) vsweep_yz_kernel(VParams P) {
     }
 }
 
-static int g_occ_x[2] = {0, 0}, g_occ_yz[2] = {0, 0};
-static size_t g_occ_x_smem[2] = {0, 0}, g_occ_yz_smem[2] = {0, 0};
+static int g_occ_x[2] = {0, 0}, g_occ_yz[4] = {0, 0, 0, 0};
+static size_t g_occ_x_smem[2] = {0, 0}, g_occ_yz_smem[4] = {0, 0, 0, 0};
 constexpr size_t V_SMEM_MAX = 200 * 1024;
 
 template <class K>
@@ -391,8 +458,9 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         P.ntot = P.ntile * ncell;
         P.nseg = (s.nv[1] + 7) / 8;
         P.nseg2 = (s.nv[2] + 7) / 8;
-        auto k = lim ? vsweep_yz_kernel<1> : vsweep_yz_kernel<0>;
-        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim], g_occ_yz_smem[lim]));
+        const bool sq32 = s.nv[0] % 2 == 0 && s.nv[1] == 32 && s.nv[2] == 32 && pt == 2;
+        auto k = sq32 ? (lim ? vsweep_yz_kernel<1, 32> : vsweep_yz_kernel<0, 32>) : (lim ? vsweep_yz_kernel<1, 0> : vsweep_yz_kernel<0, 0>);
+        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim + 2 * sq32], g_occ_yz_smem[lim + 2 * sq32]));
         Launch L(c, K_VSWEEP_YZ);
         k<<<grid, V_THREADS, smem, c->stream>>>(P);
     }
