@@ -172,16 +172,22 @@ __device__ __forceinline__ int virtual_row(const XYParams& P, int r, bool& mirro
 // rows ahead of the row being worked on.
 constexpr int XY_NS = 3;
 
-template <int XB, int LIM, int XFIRST>
+// SP > 0: nx = SP spatial cells per row, 32^3 velocity cells, the launcher's chunk for that (C = PC = 2048 / SP):
+// every stride of the kernel is a compile-time constant.  SP = 0: any shape, at run time.
+template <int XB, int LIM, int XFIRST, int SP>
 __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant__ CUtensorMap tmap, XYParams P) {
     extern __shared__ __align__(128) unsigned char smraw[];
-    const int C = P.C, C8 = C * 8;
+    constexpr int KC = SP ? 2048 / SP : 0;
+    if (SP && (P.nx != SP || P.C != KC || P.PC != KC || P.nv1 != 32 || P.nv2 != 32 || P.S != 32768)) return;
+    const int nx = SP ? SP : P.nx, nv1 = SP ? 32 : P.nv1, nv2 = SP ? 32 : P.nv2;
+    const long S = SP ? 32768 : P.S, row_stride = SP ? (long)SP * 32768 : P.row_stride;
+    const int C = SP ? KC : P.C, C8 = C * 8;
     const int c = threadIdx.x % C, blk = threadIdx.x / C;
     const int ix0 = blk * XB;
     const long v0 = (long)blockIdx.x * C;
     const long v = v0 + c;
-    const int ivx = (int)(v / ((long)P.nv1 * P.nv2));
-    const int ivy = (int)((v / P.nv2) % P.nv1);
+    const int ivx = (int)(v / ((long)nv1 * nv2));
+    const int ivy = (int)((v / nv2) % nv1);
     // the six weights of a velocity cell live in shared memory (wt[k][c]): 12 registers less per thread; only
     // the two flow directions stay in registers
     double* wt = reinterpret_cast<double*>(smraw + 128);
@@ -198,8 +204,8 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
     }
     const unsigned bar0 = smem_addr(smraw);
     // a row buffer is made of C / PC pieces, each a dense [x][PC] TMA box (128-byte aligned)
-    const int PC = P.PC, npp = C / PC, X8 = PC * 8;
-    const unsigned piecebytes = ((unsigned)P.nx * X8 + 127u) & ~127u;
+    const int PC = SP ? KC : P.PC, npp = C / PC, X8 = PC * 8;
+    const unsigned piecebytes = ((unsigned)nx * X8 + 127u) & ~127u;
     const unsigned rowbytes = piecebytes * npp;
     const unsigned raw0 = bar0 + 128 + ((6 * C * 8 + 127) & ~127);
     const unsigned hb0 = raw0 + XY_NS * rowbytes;
@@ -212,12 +218,12 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
     auto issue_row = [&](int r, int stage) {
         if (threadIdx.x == 0) {
             const unsigned bar = bar0 + 8 * stage;
-            mbar_expect_tx(bar, (unsigned)P.nx * C8);
+            mbar_expect_tx(bar, (unsigned)nx * C8);
             bool m; const int ar = virtual_row(P, r, m);
             for (int p = 0; p < npp; ++p) {
                 long vp = v0 + (long)p * PC;
-                if (m) vp += (long)(P.nv1 - 1 - 2 * (int)((vp / P.nv2) % P.nv1)) * P.nv2;
-                tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes, &tmap, (int)vp, ar * P.nx, bar);
+                if (m) vp += (long)(nv1 - 1 - 2 * (int)((vp / nv2) % nv1)) * nv2;
+                tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes, &tmap, (int)vp, ar * nx, bar);
             }
         }
     };
@@ -246,7 +252,7 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
         const unsigned sraw = raw0 + stage * rowbytes;
         mbar_wait(bar0 + 8 * stage, phase);
         const int orow = r - orow_shift;
-        double* po = P.dst + (long)(P.g + orow) * P.row_stride + (long)ix0 * P.S + v;
+        double* po = P.dst + (long)(P.g + orow) * row_stride + (long)ix0 * S + v;
         const bool store = orow >= 0 && orow < P.ny;
         const int nstage = stage == 0 ? XY_NS - 1 : stage - 1;      // stage of row r + NS - 1 = stage of row r - 1
         if (XFIRST) {
@@ -257,24 +263,24 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
             for (int k = 0; k < XB / CH; ++k) {
                 double gx[CH];
                 if (Wx.pos) {
-                    x_chunk<XB, CH, LIM, 1>(k, carry, gx, sraw, ix0, P.nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, 1>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
 #pragma unroll
                     for (int i = 0; i < CH; ++i) {
                         const int it = k * CH + i;
                         const double h = PAR == 0 ? y_step<LIM>(A[it], B[it], yG[it], gx[i], Wy, finf)
                                                   : y_step<LIM>(B[it], A[it], yG[it], gx[i], Wy, finf);
                         if (PAR == 0) A[it] = gx[i]; else B[it] = gx[i];
-                        if (store) __stcs(po + (long)it * P.S, h);
+                        if (store) __stcs(po + (long)it * S, h);
                     }
                 } else {
-                    x_chunk<XB, CH, LIM, -1>(k, carry, gx, sraw, ix0, P.nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, -1>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
 #pragma unroll
                     for (int i = 0; i < CH; ++i) {
                         const int it = XB - 1 - (k * CH + i);
                         const double h = PAR == 0 ? y_step<LIM>(A[it], B[it], yG[it], gx[i], Wy, finf)
                                                   : y_step<LIM>(B[it], A[it], yG[it], gx[i], Wy, finf);
                         if (PAR == 0) A[it] = gx[i]; else B[it] = gx[i];
-                        if (store) __stcs(po + (long)it * P.S, h);
+                        if (store) __stcs(po + (long)it * S, h);
                     }
                 }
             }
@@ -296,16 +302,16 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
             for (int k = 0; k < XB / CH; ++k) {
                 double o[CH];
                 if (Wx.pos) {
-                    x_chunk<XB, CH, LIM, 1>(k, carry, o, sh, ix0, P.nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, 1>(k, carry, o, sh, ix0, nx, X8, cofs, Wx, finf);
                     if (store) {
 #pragma unroll
-                        for (int i = 0; i < CH; ++i) __stcs(po + (long)(k * CH + i) * P.S, o[i]);
+                        for (int i = 0; i < CH; ++i) __stcs(po + (long)(k * CH + i) * S, o[i]);
                     }
                 } else {
-                    x_chunk<XB, CH, LIM, -1>(k, carry, o, sh, ix0, P.nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, -1>(k, carry, o, sh, ix0, nx, X8, cofs, Wx, finf);
                     if (store) {
 #pragma unroll
-                        for (int i = 0; i < CH; ++i) __stcs(po + (long)(XB - 1 - (k * CH + i)) * P.S, o[i]);
+                        for (int i = 0; i < CH; ++i) __stcs(po + (long)(XB - 1 - (k * CH + i)) * S, o[i]);
                     }
                 }
             }
@@ -323,15 +329,15 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
     }
 }
 
-template <int XB, int LIM>
+template <int XB, int LIM, int SP>
 static void launch_xy_t(const CUtensorMap& tm, const XYParams& P, int xfirst, dim3 grid, int threads, size_t smem,
                         cudaStream_t st) {
     if (xfirst) {
-        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        sweep_xy_kernel<XB, LIM, 1><<<grid, threads, smem, st>>>(tm, P);
+        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 1, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        sweep_xy_kernel<XB, LIM, 1, SP><<<grid, threads, smem, st>>>(tm, P);
     } else {
-        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        sweep_xy_kernel<XB, LIM, 0><<<grid, threads, smem, st>>>(tm, P);
+        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 0, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        sweep_xy_kernel<XB, LIM, 0, SP><<<grid, threads, smem, st>>>(tm, P);
     }
 }
 
@@ -424,9 +430,12 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     const int lim = G.limiter ? 1 : 0;
     {
         Launch L(c, K_SWEEP_XY);
-        if (xb == 8) { if (lim) launch_xy_t<8, 1>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<8, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
-        else if (xb == 4) { if (lim) launch_xy_t<4, 1>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
-        else { if (lim) launch_xy_t<1, 1>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        const bool v32 = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32 && xb == 4 && P.PC == C;
+        if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (v32 && G.nx == 64 && C == 32) { if (lim) launch_xy_t<4, 1, 64>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (xb == 8) { if (lim) launch_xy_t<8, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<8, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (xb == 4) { if (lim) launch_xy_t<4, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else { if (lim) launch_xy_t<1, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
     }
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }

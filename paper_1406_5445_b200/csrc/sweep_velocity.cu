@@ -272,17 +272,21 @@ constexpr int V_THREADS = 256;
 // One thread marches a segment of one column; a warp reads/writes 256 contiguous bytes per step.
 // Persistent: a CTA loops over tiles, the pad rows are zeroed once.
 // ------------------------------------------------------------------------------------------------
-template <int LIM>
+// CN > 0: a CN^3 velocity block with the launcher's tile shape for it (128 columns, 2 segments), all compile-time.
+template <int LIM, int CN>
 __global__ void __launch_bounds__(V_THREADS, 4) vsweep_x_kernel(VParams P) {
     extern __shared__ double sm[];
-    const int CT = P.ct, N = P.nv0, H = CT >> 1;
-    const int plane = P.nv1 * P.nv2;
+    if (CN && (P.ct != 128 || P.nseg != 2 || P.nv0 != CN || P.nv1 != CN || P.nv2 != CN)) return;
+    const int CT = CN ? 128 : P.ct, N = CN ? CN : P.nv0, H = CT >> 1;
+    const int nv2 = CN ? CN : P.nv2, nsegx = CN ? 2 : P.nseg;
+    const int plane = CN ? CN * CN : P.nv1 * P.nv2;
+    const int ntile = CN ? (CN * CN) / 128 : P.ntile;
     double* A = sm + 3 * CT;
     for (int e = threadIdx.x; e < 3 * CT; e += V_THREADS) { sm[e] = 0.0; A[N * CT + e] = 0.0; }
-    const int seglen = (N + P.nseg - 1) / P.nseg;
+    const int seglen = (N + nsegx - 1) / nsegx;
     for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x) {
-        const int cell = P.cell0 + tile / P.ntile;
-        const int c0 = (tile % P.ntile) * CT;
+        const int cell = P.cell0 + tile / ntile;
+        const int c0 = (tile % ntile) * CT;
         const int ncol = min(CT, plane - c0);
         const double* T = P.table + (long)cell * TAB;
         const double t0 = T[0], t1 = T[1], t2 = T[2], t3 = T[3], finf = T[12], scale = T[15];
@@ -295,11 +299,11 @@ __global__ void __launch_bounds__(V_THREADS, 4) vsweep_x_kernel(VParams P) {
             *reinterpret_cast<double2*>(A + k * CT + c) = v;
         }
         __syncthreads();
-        for (int wi = threadIdx.x; wi < CT * P.nseg; wi += V_THREADS) {
+        for (int wi = threadIdx.x; wi < CT * nsegx; wi += V_THREADS) {
             const int seg = wi / CT, c = wi - seg * CT;
             if (c < ncol) {
                 const int col = c0 + c;
-                const int k1 = col / P.nv2, k2 = col - k1 * P.nv2;
+                const int k1 = col / nv2, k2 = col - k1 * nv2;
                 const double s0 = t0 + t2 * k1 + t3 * k2;
                 const int a = seg * seglen, b = min(a + seglen, N);
                 OutGlobal o{fb + c + (long)a * plane, (long)plane};
@@ -402,8 +406,8 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
     }
 }
 
-static int g_occ_x[2] = {0, 0}, g_occ_yz[4] = {0, 0, 0, 0};
-static size_t g_occ_x_smem[2] = {0, 0}, g_occ_yz_smem[4] = {0, 0, 0, 0};
+static int g_occ_x[4] = {0, 0, 0, 0}, g_occ_yz[4] = {0, 0, 0, 0};
+static size_t g_occ_x_smem[4] = {0, 0, 0, 0}, g_occ_yz_smem[4] = {0, 0, 0, 0};
 constexpr size_t V_SMEM_MAX = 200 * 1024;
 
 template <class K>
@@ -438,8 +442,9 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         P.ntile = (plane + ct - 1) / ct;
         P.ntot = P.ntile * ncell;
         P.nseg = V_THREADS / ct; if (P.nseg < 1) P.nseg = 1; if (P.nseg > s.nv[0]) P.nseg = s.nv[0];
-        auto k = lim ? vsweep_x_kernel<1> : vsweep_x_kernel<0>;
-        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim], g_occ_x_smem[lim]));
+        const bool cube32 = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32 && ct == 128 && P.nseg == 2;
+        auto k = cube32 ? (lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>) : (lim ? vsweep_x_kernel<1, 0> : vsweep_x_kernel<0, 0>);
+        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim + 2 * cube32], g_occ_x_smem[lim + 2 * cube32]));
         Launch L(c, K_VSWEEP_X);
         k<<<grid, V_THREADS, smem, c->stream>>>(P);
     }
