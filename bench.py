@@ -33,7 +33,7 @@ UNIT = "cell-updates/s"
 
 # Algorithmic HBM bytes per phase-space cell and launch of each f-sized kernel:
 # a sweep reads and writes every cell once (8 + 8 B); the moments pass reads it once.
-BYTES_PER_CELL = {"sweep_x": 16.0, "sweep_y": 16.0, "sweep_xy": 16.0, "vsweep_x": 16.0, "vsweep_yz": 16.0,
+BYTES_PER_CELL = {"sweep_x": 16.0, "sweep_y": 16.0, "sweep_xy": 16.0, "sweep_yx": 16.0, "vsweep_x": 16.0, "vsweep_yz": 16.0,
                   "vsweep_xyz": 16.0, "moments": 8.0}
 
 

@@ -429,7 +429,7 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     const int threads = nblk * C;
     const int lim = G.limiter ? 1 : 0;
     {
-        Launch L(c, K_SWEEP_XY);
+        Launch L(c, xfirst ? K_SWEEP_XY : K_SWEEP_YX);
         const bool v32 = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32 && xb == 4 && P.PC == C;
         if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (v32 && G.nx == 64 && C == 32) { if (lim) launch_xy_t<4, 1, 64>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64>(tm, P, xfirst, grid, threads, smem, c->stream); }

@@ -67,7 +67,7 @@ struct vlasov_ctx {
 namespace vl {
 
 enum Kind { K_SWEEP_X = 0, K_SWEEP_Y, K_TABLE, K_VSWEEP_X, K_VSWEEP_YZ, K_MOMENTS, K_GHOST_TABLE, K_CURRENT,
-            K_MAXWELL, K_SWEEP_XY, K_COUNT };
+            K_MAXWELL, K_SWEEP_XY, K_SWEEP_YX, K_COUNT };
 
 // Counts a launch and, when timing is on, brackets it with an event pair on the context's stream.
 struct Launch {

@@ -131,14 +131,15 @@ def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
     dt = 0.05          # |sigma_x| <= 4 * 0.025 / (1.7/24) = 0.71 ... 0.38; |sigma_y| <= 3 * 0.025 / (0.9/7) = 0.58
     fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, Z, Z, dt, stages, fuse=1)
     assert code == 0
-    assert run_both.kinds["sweep_xy"][1] == 1 and run_both.kinds["sweep_y"][1] == 0      # the fused kernel ran
+    fused = run_both.kinds["sweep_xy" if stages == 1 else "sweep_yx"][1]
+    assert fused == 1 and run_both.kinds["sweep_y"][1] == 0                              # the fused kernel ran
     assert run_both.kinds["sweep_x"][1] == (2 if g else 0)                               # ghost rows: x sweep only
     assert rel_l2(fg[0], fo[0]) <= TOL1
     assert np.abs(fg[0] - fo[0]).max() <= 1e-13
     assert rel_l2(mg[0], mo[0]) <= TOL1
     fu, _, _, _, code = run_both(gpu, orc, w, f0, Z, Z, dt, stages, fuse=0)
     assert code == 0
-    assert run_both.kinds["sweep_xy"][1] == 0 and run_both.kinds["sweep_y"][1] == 1
+    assert run_both.kinds["sweep_xy"][1] + run_both.kinds["sweep_yx"][1] == 0 and run_both.kinds["sweep_y"][1] == 1
     assert rel_l2(fg[0], fu[0]) <= TOL1
 
 
@@ -405,7 +406,7 @@ def test_full_size_gem128_sampled_window(gpu, orc):
     ctx.vlasov_step(w.dt, Ed, Bd, gpu.STAGE_ALL)
     assert ctx.check_code() == 0
     kinds = ctx.vlasov_timing_read()
-    assert kinds["sweep_xy"][1] == 4 and kinds["vsweep_yz"][1] == 2        # the configuration bench.py times
+    assert kinds["sweep_xy"][1] == 2 and kinds["sweep_yx"][1] == 2 and kinds["vsweep_yz"][1] == 2   # as bench.py times it
     Ew = np.ascontiguousarray(E[:, iy0:iy0 + nw, ix0:ix0 + nw])
     Bw = np.ascontiguousarray(B[:, iy0:iy0 + nw, ix0:ix0 + nw])
     inner = slice(margin, nw - margin)
