@@ -334,21 +334,21 @@ struct VParams {
 constexpr int V_THREADS = 256;
 
 // ------------------------------------------------------------------------------------------------
-// a4: vx sweep.  Tile = all i_vx x CT contiguous (i_vy,i_vz) columns, rows -3..-1 and N..N+2 zero.
+// a4: vx sweep.  Tile = all i_vx x CT contiguous (i_vy,i_vz) columns, rows -V_PAD..-1 and N..N+V_PAD-1 zero.
 // One thread marches a segment of one column; a warp reads/writes 256 contiguous bytes per step.
 // Persistent: a CTA loops over tiles, the pad rows are zeroed once.
 // ------------------------------------------------------------------------------------------------
 // CN > 0: a CN^3 velocity block with the launcher's tile shape for it (128 columns, 2 segments), all compile-time.
 template <int LIM, int CN>
-__global__ void __launch_bounds__(V_THREADS, 4) vsweep_x_kernel(VParams P) {
+__global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams P) {
     extern __shared__ double sm[];
-    if (CN && (P.ct != 128 || P.nseg != 2 || P.nv0 != CN || P.nv1 != CN || P.nv2 != CN)) return;
+    if (CN && (P.ct != 128 || P.nseg != CN / 8 || P.nv0 != CN || P.nv1 != CN || P.nv2 != CN)) return;
     const int CT = CN ? 128 : P.ct, N = CN ? CN : P.nv0, H = CT >> 1;
-    const int nv2 = CN ? CN : P.nv2, nsegx = CN ? 2 : P.nseg;
+    const int nv2 = CN ? CN : P.nv2, nsegx = CN ? CN / 8 : P.nseg;
     const int plane = CN ? CN * CN : P.nv1 * P.nv2;
     const int ntile = CN ? (CN * CN) / 128 : P.ntile;
-    double* A = sm + 3 * CT;
-    for (int e = threadIdx.x; e < 3 * CT; e += V_THREADS) { sm[e] = 0.0; A[N * CT + e] = 0.0; }
+    double* A = sm + V_PAD * CT;
+    for (int e = threadIdx.x; e < V_PAD * CT; e += V_THREADS) { sm[e] = 0.0; A[N * CT + e] = 0.0; }
     const int seglen = (N + nsegx - 1) / nsegx;
     for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x) {
         const int cell = P.cell0 + tile / ntile;
@@ -373,7 +373,7 @@ __global__ void __launch_bounds__(V_THREADS, 4) vsweep_x_kernel(VParams P) {
                 const double s0 = t0 + t2 * k1 + t3 * k2;
                 const int a = seg * seglen, b = min(a + seglen, N);
                 OutGlobal o{fb + c + (long)a * plane, (long)plane};
-                march_cells<LIM, 0>(smem_addr(A + c), CT * 8, N, a, b, s0, t1, finf, o);
+                march_cells<LIM, (CN ? 1 : 0)>(smem_addr(A + c), CT * 8, N, a, b, s0, t1, finf, o);
             }
         }
         __syncthreads();
@@ -500,15 +500,17 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
     const int ncell = nrows * c->G.nx;
     const int plane = s.nv[1] * s.nv[2];
     {
+        const bool cube = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32;
         int ct = 128;
-        while (ct > 32 && ((size_t)(s.nv[0] + 6) * ct * 8 > 48 * 1024 || ct / 2 >= plane)) ct >>= 1;
+        while (ct > 32 && ((size_t)(s.nv[0] + 2 * V_PAD) * ct * 8 > 48 * 1024 || ct / 2 >= plane)) ct >>= 1;
         P.ct = ct;
-        const size_t smem = (size_t)(s.nv[0] + 6) * ct * 8;
+        const size_t smem = (size_t)(s.nv[0] + 2 * V_PAD) * ct * 8;
         if (smem > V_SMEM_MAX) return VLASOV_EINVAL;
         P.ntile = (plane + ct - 1) / ct;
         P.ntot = P.ntile * ncell;
         P.nseg = V_THREADS / ct; if (P.nseg < 1) P.nseg = 1; if (P.nseg > s.nv[0]) P.nseg = s.nv[0];
-        const bool cube32 = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32 && ct == 128 && P.nseg == 2;
+        if (cube && ct == 128) P.nseg = 4;                 // 8-cell segments (register-window walk), two per thread and tile
+        const bool cube32 = cube && ct == 128 && P.nseg == 4;
         auto k = cube32 ? (lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>) : (lim ? vsweep_x_kernel<1, 0> : vsweep_x_kernel<0, 0>);
         const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim + 2 * cube32], g_occ_x_smem[lim + 2 * cube32]));
         Launch L(c, K_VSWEEP_X);

@@ -169,20 +169,30 @@ __device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, dou
     sp = dp; sm = dm;
     if (LIM) {
         const double g = finf - f0;
-        const int hb = min(__double2hiint(f0), __double2hiint(g)) + 0x00100000;
+        const int hf = __double2hiint(f0) + 0x00100000, hg = __double2hiint(g) + 0x00100000;
         const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
-        const bool need = max(hp, hm) >= hb;
-        if (__any_sync(__activemask(), need)) {
-            const double hiA = relu_bits(f0 + f0), hiB = relu_bits(g + g);
-            const bool pneg = __double2hiint(dp) < 0, mneg = __double2hiint(dm) < 0;
-            const double bp = pneg ? hiB : hiA;
-            const double bm = mneg ? hiA : hiB;
-            const double ap = __hiloint2double(hp, __double2loint(dp));      // |d+|
-            const double am = __hiloint2double(hm, __double2loint(dm));      // |d-|
-            const double mp = ap < bp ? ap : bp;
-            const double mm = am < bm ? am : bm;
-            sp = __hiloint2double(__double2hiint(mp) | (__double2hiint(dp) & 0x80000000), __double2loint(mp));
-            sm = __hiloint2double(__double2hiint(mm) | (__double2hiint(dm) & 0x80000000), __double2loint(mm));
+        const int hmax = max(hp, hm);
+        const unsigned mask = __activemask();
+        if (__any_sync(mask, hmax >= min(hf, hg))) {
+            const double hiA = relu_bits(f0 + f0);
+            if (!__any_sync(mask, hmax >= hg)) {
+                // only the positivity bound 2 f0 can bind (the tails of a distribution, far below f_inf):
+                // eps+ d+ = min(d+, hiA), eps- d- = max(d-, -hiA)
+                const double nA = -hiA;
+                sp = dp < hiA ? dp : hiA;
+                sm = dm > nA ? dm : nA;
+            } else {
+                const double hiB = relu_bits(g + g);
+                const bool pneg = __double2hiint(dp) < 0, mneg = __double2hiint(dm) < 0;
+                const double bp = pneg ? hiB : hiA;
+                const double bm = mneg ? hiA : hiB;
+                const double ap = __hiloint2double(hp, __double2loint(dp));      // |d+|
+                const double am = __hiloint2double(hm, __double2loint(dm));      // |d-|
+                const double mp = ap < bp ? ap : bp;
+                const double mm = am < bm ? am : bm;
+                sp = __hiloint2double(__double2hiint(mp) | (__double2hiint(dp) & 0x80000000), __double2loint(mp));
+                sm = __hiloint2double(__double2hiint(mm) | (__double2hiint(dm) & 0x80000000), __double2loint(mm));
+            }
         }
     }
 }
