@@ -354,7 +354,18 @@ def gpu_arm(args):
             if tj.get("workload") == w.name and dom in tj.get("dram_bytes_per_launch", {}):
                 roofline["traffic"] = tj["dram_bytes_per_launch"][dom]
                 roofline["traffic_source"] = tj.get("source")
-    pass_bytes = sum(BYTES_PER_CELL[k] * v["launches_per_step"] / ns for k, v in kinds.items() if k in BYTES_PER_CELL)
+    # f-sized passes of one step and species.  With FLUID sides some launches of a kind cover only ghost rows (the
+    # ghost fill's velocity sweeps and edge-row moments, the x sweep of the ghost rows beside a fused stage): a kind
+    # counts once per species there, and the one-direction sweeps only when no fused stage ran.
+    fused = any(k in kinds for k in ("sweep_xy", "sweep_yx"))
+
+    def full_passes(k, v):
+        n = v["launches_per_step"] / ns
+        if k in ("sweep_x", "sweep_y"):
+            return 0.0 if fused else n
+        return min(n, 1.0) if fluid is not None else n
+
+    pass_bytes = sum(BYTES_PER_CELL[k] * full_passes(k, v) for k, v in kinds.items() if k in BYTES_PER_CELL)
 
     # ---- the oracle timed beside it (reported baseline only) --------------------------------
     cpu = None
