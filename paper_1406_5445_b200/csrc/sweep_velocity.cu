@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams
     const int CT = CN ? 128 : P.ct, N = CN ? CN : P.nv0, H = CT >> 1;
     const int nv2 = CN ? CN : P.nv2, nsegx = CN ? CN / 8 : P.nseg;
     const int plane = CN ? CN * CN : P.nv1 * P.nv2;
-    const int ntile = CN ? (CN * CN) / 128 : P.ntile;
+    const int ntile = CN ? (CN * CN + 127) / 128 : P.ntile;
     double* A = sm + V_PAD * CT;
     for (int e = threadIdx.x; e < V_PAD * CT; e += V_THREADS) { sm[e] = 0.0; A[N * CT + e] = 0.0; }
     const int seglen = (N + nsegx - 1) / nsegx;
@@ -392,7 +392,7 @@ template <int LIM, int CN>
 __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
     extern __shared__ double sm[];
     const int N1 = CN ? CN : P.nv1, N2 = CN ? CN : P.nv2;
-    constexpr int CCT = CN ? (8 * V_THREADS) / (CN * CN) : 0;      // planes per tile, as launch_vsweeps picks them
+    constexpr int CCT = CN ? ((8 * V_THREADS) / (CN * CN) > 0 ? (8 * V_THREADS) / (CN * CN) : 1) : 0;      // planes per tile, as launch_vsweeps picks them
     constexpr int CSEG = CN ? (CN + 7) / 8 : 0;
     if (CN && (P.ct != CCT || P.nseg != CSEG || P.nseg2 != CSEG)) return;
     const int ct = CN ? CCT : P.ct, nseg1 = CN ? CSEG : P.nseg, nseg2 = CN ? CSEG : P.nseg2;
@@ -500,7 +500,8 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
     const int ncell = nrows * c->G.nx;
     const int plane = s.nv[1] * s.nv[2];
     {
-        const bool cube = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32;
+        const int cn = (s.nv[0] == s.nv[1] && s.nv[1] == s.nv[2]) ? s.nv[0] : 0;
+        const bool cube = cn == 16 || cn == 32;            // shapes with a compile-time-shape kernel
         int ct = 128;
         while (ct > 32 && ((size_t)(s.nv[0] + 2 * V_PAD) * ct * 8 > 48 * 1024 || ct / 2 >= plane)) ct >>= 1;
         P.ct = ct;
@@ -509,9 +510,12 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         P.ntile = (plane + ct - 1) / ct;
         P.ntot = P.ntile * ncell;
         P.nseg = V_THREADS / ct; if (P.nseg < 1) P.nseg = 1; if (P.nseg > s.nv[0]) P.nseg = s.nv[0];
-        if (cube && ct == 128) P.nseg = 4;                 // 8-cell segments (register-window walk), two per thread and tile
-        const bool cube32 = cube && ct == 128 && P.nseg == 4;
-        auto k = cube32 ? (lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>) : (lim ? vsweep_x_kernel<1, 0> : vsweep_x_kernel<0, 0>);
+        if (cube && ct == 128) P.nseg = cn / 8;            // 8-cell segments (register-window walk)
+        const int spec = (cube && ct == 128) ? cn : 0;
+        void (*k)(VParams) = lim ? vsweep_x_kernel<1, 0> : vsweep_x_kernel<0, 0>;
+        if (spec == 16) k = lim ? vsweep_x_kernel<1, 16> : vsweep_x_kernel<0, 16>;
+        if (spec == 32) k = lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>;
+        const int cube32 = spec ? 1 : 0;
         const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim + 2 * cube32], g_occ_x_smem[lim + 2 * cube32]));
         Launch L(c, K_VSWEEP_X);
         k<<<grid, V_THREADS, smem, c->stream>>>(P);
@@ -531,8 +535,16 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         P.ntot = P.ntile * ncell;
         P.nseg = (s.nv[1] + 7) / 8;
         P.nseg2 = (s.nv[2] + 7) / 8;
-        const bool sq32 = s.nv[0] % 2 == 0 && s.nv[1] == 32 && s.nv[2] == 32 && pt == 2;
-        auto k = sq32 ? (lim ? vsweep_yz_kernel<1, 32> : vsweep_yz_kernel<0, 32>) : (lim ? vsweep_yz_kernel<1, 0> : vsweep_yz_kernel<0, 0>);
+        const int sq = s.nv[1] == s.nv[2] ? s.nv[1] : 0;   // square planes with a compile-time-shape kernel
+        const int want_pt = sq ? ((8 * V_THREADS) / (sq * sq) > 0 ? (8 * V_THREADS) / (sq * sq) : 1) : 0;
+        const int spec = (sq == 16 || sq == 24 || sq == 32 || sq == 40 || sq == 48) && pt == want_pt ? sq : 0;
+        void (*k)(VParams) = lim ? vsweep_yz_kernel<1, 0> : vsweep_yz_kernel<0, 0>;
+        if (spec == 16) k = lim ? vsweep_yz_kernel<1, 16> : vsweep_yz_kernel<0, 16>;
+        if (spec == 24) k = lim ? vsweep_yz_kernel<1, 24> : vsweep_yz_kernel<0, 24>;
+        if (spec == 32) k = lim ? vsweep_yz_kernel<1, 32> : vsweep_yz_kernel<0, 32>;
+        if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
+        if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
+        const int sq32 = spec ? 1 : 0;
         const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim + 2 * sq32], g_occ_yz_smem[lim + 2 * sq32]));
         Launch L(c, K_VSWEEP_YZ);
         k<<<grid, V_THREADS, smem, c->stream>>>(P);
