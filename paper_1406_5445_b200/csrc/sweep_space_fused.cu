@@ -153,6 +153,29 @@ __device__ __forceinline__ double y_step(double ya, double yb, double& yG, doubl
     return h;
 }
 
+// NB steps of the y march at once (the owned cells of one x chunk): one limiter vote for all of them, so that the
+// NB flux evaluations are independent instruction streams.
+template <int NB, int LIM>
+__device__ __forceinline__ void y_batch(const double (&ya)[NB], const double (&yb)[NB], double (&yG)[NB],
+                                        const double (&gx)[NB], const Weights& Wy, double finf, double (&h)[NB]) {
+    double dlo[NB], dhi[NB];
+    int need = 0;
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+        dlo[i] = yb[i] - ya[i]; dhi[i] = gx[i] - yb[i];
+        if (LIM) need |= need_bits(yb[i], dhi[i], dlo[i], finf);
+    }
+    const bool slow = LIM && __any_sync(__activemask(), need < 0);
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+        double sp = Wy.pos ? dhi[i] : -dlo[i], sm = Wy.pos ? dlo[i] : -dhi[i];
+        if (slow) { if (Wy.pos) slopes_fast<1>(ya[i], yb[i], gx[i], finf, sp, sm); else slopes_fast<1>(gx[i], yb[i], ya[i], finf, sp, sm); }
+        const double Gn = fma(Wy.w2, sm, fma(Wy.w1, sp, Wy.w0 * yb[i]));
+        h[i] = Wy.pos ? yb[i] + (yG[i] - Gn) : ya[i] + (Gn - yG[i]);
+        yG[i] = Gn;
+    }
+}
+
 // Array row and image flag of boundary-inclusive row r (-2 <= r <= ny+1) of the y sweep.
 __device__ __forceinline__ int virtual_row(const XYParams& P, int r, bool& mirror) {
     mirror = false;
@@ -264,36 +287,45 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
                 double gx[CH];
                 if (Wx.pos) {
                     x_chunk<XB, CH, LIM, 1>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
+                    double ya[CH], yb[CH], g[CH], h[CH];
+#pragma unroll
+                    for (int i = 0; i < CH; ++i) { const int it = k * CH + i; ya[i] = PAR == 0 ? A[it] : B[it]; yb[i] = PAR == 0 ? B[it] : A[it]; g[i] = yG[it]; }
+                    y_batch<CH, LIM>(ya, yb, g, gx, Wy, finf, h);
 #pragma unroll
                     for (int i = 0; i < CH; ++i) {
                         const int it = k * CH + i;
-                        const double h = PAR == 0 ? y_step<LIM>(A[it], B[it], yG[it], gx[i], Wy, finf)
-                                                  : y_step<LIM>(B[it], A[it], yG[it], gx[i], Wy, finf);
+                        yG[it] = g[i];
                         if (PAR == 0) A[it] = gx[i]; else B[it] = gx[i];
-                        if (store) __stcs(po + (long)it * S, h);
+                        if (store) __stcs(po + (long)it * S, h[i]);
                     }
                 } else {
                     x_chunk<XB, CH, LIM, -1>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
+                    double ya[CH], yb[CH], g[CH], h[CH];
+#pragma unroll
+                    for (int i = 0; i < CH; ++i) { const int it = XB - 1 - (k * CH + i); ya[i] = PAR == 0 ? A[it] : B[it]; yb[i] = PAR == 0 ? B[it] : A[it]; g[i] = yG[it]; }
+                    y_batch<CH, LIM>(ya, yb, g, gx, Wy, finf, h);
 #pragma unroll
                     for (int i = 0; i < CH; ++i) {
                         const int it = XB - 1 - (k * CH + i);
-                        const double h = PAR == 0 ? y_step<LIM>(A[it], B[it], yG[it], gx[i], Wy, finf)
-                                                  : y_step<LIM>(B[it], A[it], yG[it], gx[i], Wy, finf);
+                        yG[it] = g[i];
                         if (PAR == 0) A[it] = gx[i]; else B[it] = gx[i];
-                        if (store) __stcs(po + (long)it * S, h);
+                        if (store) __stcs(po + (long)it * S, h[i]);
                     }
                 }
             }
             __syncthreads();                       // everybody is done reading raw row r
         } else {
             const unsigned sh = hb0 + (unsigned)PAR * rowbytes;
+            {
+                double gx[XB], h[XB];
 #pragma unroll
-            for (int i = 0; i < XB; ++i) {
-                const double gx = lds(sraw + own + i * X8);
-                const double h = PAR == 0 ? y_step<LIM>(A[i], B[i], yG[i], gx, Wy, finf)
-                                          : y_step<LIM>(B[i], A[i], yG[i], gx, Wy, finf);
-                if (PAR == 0) A[i] = gx; else B[i] = gx;
-                sts(sh + own + i * X8, h);
+                for (int i = 0; i < XB; ++i) gx[i] = lds(sraw + own + i * X8);
+                if (PAR == 0) y_batch<XB, LIM>(A, B, yG, gx, Wy, finf, h); else y_batch<XB, LIM>(B, A, yG, gx, Wy, finf, h);
+#pragma unroll
+                for (int i = 0; i < XB; ++i) {
+                    if (PAR == 0) A[i] = gx[i]; else B[i] = gx[i];
+                    sts(sh + own + i * X8, h[i]);
+                }
             }
             __syncthreads();                       // y-swept row complete; raw rows up to r are free
             if (r + XY_NS <= rlast) issue_row(r + XY_NS, stage);
