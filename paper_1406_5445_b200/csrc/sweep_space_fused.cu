@@ -191,9 +191,9 @@ __device__ __forceinline__ int virtual_row(const XYParams& P, int r, bool& mirro
 
 // XFIRST = 1: x remap of every incoming row, then the y march (a1 + a2).
 // XFIRST = 0: y march on the raw rows, then the x remap of every finished row (a7 + a8).
-// Shared memory: [NS mbarriers][NS raw rows]([2 y-swept rows] if !XFIRST).  Raw rows arrive by bulk TMA, NS - 1
+// Shared memory: [NS mbarriers][NS raw rows]([2 y-swept rows] if !XFIRST).  Raw rows arrive by tiled TMA, NS - 1
 // rows ahead of the row being worked on.
-constexpr int XY_NS = 3;
+constexpr int XY_NS = 5;
 
 // SP > 0: nx = SP spatial cells per row, 32^3 velocity cells, the launcher's chunk for that (C = PC = 2048 / SP):
 // every stride of the kernel is a compile-time constant.  SP = 0: any shape, at run time.
