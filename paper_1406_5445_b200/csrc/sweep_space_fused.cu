@@ -8,9 +8,11 @@
 // spatial cell and marches over the rows (y) of the block:
 //   * a thread owns XB consecutive x cells of one velocity cell; its warp reads/writes C*8 contiguous
 //     bytes per (x, y);
-//   * x couples threads: the row's values go through a double-buffered shared row [x][c] and each thread
-//     reads the 3 halo cells of its x block (periodic wrap);
-//   * y is private to a thread: a 2-cell register window plus the previous flux per owned cell.
+//   * raw rows arrive by 2D tiled TMA into a ring of shared rows [x][c], several rows ahead of the compute;
+//   * x couples threads: each thread reads its cells and the 3 halo cells of its x block from the shared row
+//     (periodic wrap);
+//   * y is private to a thread: a 2-row register window (the two arrays swap roles every row) plus the
+//     previous flux per owned cell.
 // Rows -2, -1 and ny, ny+1 are the boundary rows of the y sweep (R16, R19): periodic wrap, the wall
 // image f(y_w + eta, vy) = f(y_w - eta, -vy), or FLUID ghost rows; they are loaded like any row.
 #include <cstdlib>
@@ -35,7 +37,7 @@ struct XYParams {
     int bc_lo, bc_hi;
 };
 
-// ---- 1D bulk TMA (cp.async.bulk) + mbarrier: rows land in shared memory without passing registers ----
+// ---- mbarriers and tiled TMA: rows land in shared memory without passing registers ----
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
@@ -53,11 +55,6 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "DONE:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-
 // 2D tiled TMA: box {PC cells, nx spatial cells} of row `c1 / nx` lands dense in shared memory as [x][PC]
 __device__ __forceinline__ void tma_g2s_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
@@ -114,9 +111,6 @@ __device__ __forceinline__ void flux_line(const double (&q)[N + 2], const Weight
 // sbuf ([x][c], this thread's column at byte offset cofs).  DIR = +1: sigma >= 0, eq. (46); DIR = -1: eq. (47),
 // the same on the mirrored line.  val[i] = new average, eq. (38), of owned cell item(k, i); the flux through
 // the chunk border is carried over (same arithmetic on the same inputs: identical value).
-template <int XB, int CH, int DIR>
-__device__ __forceinline__ int x_item(int k, int i) { return DIR > 0 ? k * CH + i : XB - 1 - (k * CH + i); }
-
 template <int XB, int CH, int LIM, int DIR>
 __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH], unsigned sbuf, int ix0, int nx, int C8,
                                         unsigned cofs, const Weights& W, double finf) {
@@ -136,25 +130,9 @@ __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH],
     for (int i = 0; i < CH; ++i) val[i] = q[i + 2] + (G[i] - G[i + 1]);
 }
 
-// One step of the y march of an owned cell: rows (r-2, r-1, r) = (ya, yb, gx) -> new average h of row r-1
-// (sigma_y >= 0, eq. 46) or r-2 (sigma_y < 0, eq. 47 on the mirrored line).
-template <int LIM>
-__device__ __forceinline__ double y_step(double ya, double yb, double& yG, double gx, const Weights& Wy, double finf) {
-    const double dlo = yb - ya, dhi = gx - yb;
-    double sp = Wy.pos ? dhi : -dlo, sm = Wy.pos ? dlo : -dhi;
-    if (LIM) {
-        if (__any_sync(__activemask(), need_bits(yb, dhi, dlo, finf) < 0)) {
-            if (Wy.pos) slopes_fast<1>(ya, yb, gx, finf, sp, sm); else slopes_fast<1>(gx, yb, ya, finf, sp, sm);
-        }
-    }
-    const double Gn = fma(Wy.w2, sm, fma(Wy.w1, sp, Wy.w0 * yb));
-    const double h = Wy.pos ? yb + (yG - Gn) : ya + (Gn - yG);
-    yG = Gn;
-    return h;
-}
-
-// NB steps of the y march at once (the owned cells of one x chunk): one limiter vote for all of them, so that the
-// NB flux evaluations are independent instruction streams.
+// NB steps of the y march at once (the owned cells of one x chunk): rows (r-2, r-1, r) = (ya, yb, gx) -> new average
+// h of row r-1 (sigma_y >= 0, eq. 46) or r-2 (sigma_y < 0, eq. 47 on the mirrored line).  One limiter vote for all
+// NB of them, so that the flux evaluations are independent instruction streams.
 template <int NB, int LIM>
 __device__ __forceinline__ void y_batch(const double (&ya)[NB], const double (&yb)[NB], double (&yG)[NB],
                                         const double (&gx)[NB], const Weights& Wy, double finf, double (&h)[NB]) {

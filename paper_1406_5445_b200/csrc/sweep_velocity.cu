@@ -310,14 +310,6 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
     if (b == N) out.put(lds(ci) + phi_lo);           // zero flux through the upper box face (R7)
 }
 
-// q = e / d, r = e % d with m = floor((2^32 - 1) / d): the estimate is at most 2 short.
-__device__ __forceinline__ void fast_divmod(unsigned e, unsigned d, unsigned m, unsigned& q, unsigned& r) {
-    q = __umulhi(e, m);
-    r = e - q * d;
-    if (r >= d) { r -= d; ++q; }
-    if (r >= d) { r -= d; ++q; }
-}
-
 struct VParams {
     double* __restrict__ f;
     const double* __restrict__ table;

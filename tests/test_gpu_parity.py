@@ -424,3 +424,36 @@ def test_full_size_gem128_sampled_window(gpu, orc):
         # and the window's own edge does differ (the comparison is not vacuous)
         assert rel_l2(got[0], fo[0]) > 1e-9
     ctx.close()
+
+
+def test_gem_cut_50_cycles(gpu, orc):
+    """north_star's long bar on a cut of config 2 (GEM Harris sheet, both species, 50 steps): 50 full cycles of
+    section 4.3 (currents -> Maxwell half step -> Vlasov step -> currents -> Maxwell half step) through vlasov_cycle
+    against the same cycle composed from the oracle's functions: relative L2 <= 1e-10 on f, fields and moments,
+    relative mass drift <= 1e-13 per species."""
+    import os
+    import sys
+    import torch
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    w = inputs.gem_workload(nx=16, ny=8, nv=16, steps=50)
+    ref = bench.OracleRun(w)                       # sets f_inf of the species, builds f, E, B, initial moments
+    fg = [dev(f) for f in ref.f]
+    mass0 = [float(f.sum()) for f in ref.f]
+    ctx = gpu.context_for(w, fg)
+    Ed, Bd = dev(ref.E), dev(ref.B)
+    for _ in range(50):
+        ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+        ref.cycle()
+    assert ctx.check_code() == 0
+    assert rel_l2(Ed.cpu().numpy(), ref.E) <= TOL50
+    assert rel_l2(Bd.cpu().numpy(), ref.B) <= TOL50
+    mom = torch.empty((10, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+    for s in range(2):
+        got = fg[s].cpu().numpy()
+        assert rel_l2(got, ref.f[s]) <= TOL50, s
+        ctx.vlasov_moments(s, mom)
+        assert rel_l2(mom.cpu().numpy(), ref.mom[s]) <= TOL50, s
+        assert abs(float(got.sum()) - mass0[s]) / mass0[s] <= 1e-13, s
+        assert np.abs(got - inputs.gem_f(w, s)).max() > 1e-6 * got.max()         # 50 steps did move things
+    ctx.close()
