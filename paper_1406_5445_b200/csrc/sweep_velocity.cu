@@ -387,6 +387,10 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
     constexpr int CCT = CN ? ((8 * V_THREADS) / (CN * CN) > 0 ? (8 * V_THREADS) / (CN * CN) : 1) : 0;      // planes per tile, as launch_vsweeps picks them
     constexpr int CSEG = CN ? (CN + 7) / 8 : 0;
     if (CN && (P.ct != CCT || P.nseg != CSEG || P.nseg2 != CSEG)) return;
+    // REGULAR: a thread's cells of a tile are DROW whole rows apart and a row index never wraps inside a plane step:
+    // every staging offset is a compile-time constant (32x32 and 16x16 planes with 256 threads)
+    constexpr int DROW = CN ? V_THREADS / CN : 1;
+    constexpr bool REGULAR = CN && V_THREADS % (CN ? CN : 1) == 0 && (CN ? CN : 1) % DROW == 0;
     const int ct = CN ? CCT : P.ct, nseg1 = CN ? CSEG : P.nseg, nseg2 = CN ? CSEG : P.nseg2;
     const int plane = N1 * N2;
     const int RS = N2 + V_PAD, PS = (N1 + V_PAD) * RS, OFF = V_PAD * RS + V_PAD;
@@ -410,7 +414,12 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
         double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
         const double* T = P.table + (long)cell * TAB;
         const int ncellt = np * plane;
-        {   // global -> A by 8-byte cp.async; (pp, y, z) of e = threadIdx.x + i V_THREADS advanced by carries
+        if (REGULAR) {   // global -> A by 8-byte cp.async: element i of this thread sits DROW rows further, all offsets constant
+#pragma unroll
+            for (int i = 0; i < (CN ? CCT * CN * CN / V_THREADS : 1); ++i)
+                cp_async8(sA + (so_init + ((i * DROW) / (CN ? CN : 1)) * PS + ((i * DROW) % (CN ? CN : 1)) * RS) * 8, fb + threadIdx.x + i * V_THREADS);
+            cp_async_wait_all();
+        } else {   // (pp, y, z) of e = threadIdx.x + i V_THREADS advanced by carries
             int z = z_init, y = y_init;
             unsigned so = so_init;
             for (int e = threadIdx.x; e < ncellt; e += V_THREADS) {
@@ -450,7 +459,11 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
             }
         }
         __syncthreads();
-        {
+        if (REGULAR) {
+#pragma unroll
+            for (int i = 0; i < (CN ? CCT * CN * CN / V_THREADS : 1); ++i)
+                __stcs(fb + threadIdx.x + i * V_THREADS, lds(sA + (so_init + ((i * DROW) / (CN ? CN : 1)) * PS + ((i * DROW) % (CN ? CN : 1)) * RS) * 8));
+        } else {
             int z = z_init, y = y_init;
             unsigned so = so_init;
             for (int e = threadIdx.x; e < ncellt; e += V_THREADS) {
