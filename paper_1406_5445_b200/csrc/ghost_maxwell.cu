@@ -85,7 +85,7 @@ int launch_ghost_fill(vlasov_ctx* c, const Species& s, double* f, int side) {
         ghost_table_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(P);
     }
     if (cudaGetLastError() != cudaSuccess) return VLASOV_ECUDA;
-    return launch_vsweeps(c, s, f, side == 0 ? 0 : G.g + G.ny, G.g);
+    return launch_vsweeps(c, s, f, side == 0 ? 0 : G.g + G.ny, G.g, true);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -17,8 +17,8 @@
 // image f(y_w + eta, vy) = f(y_w - eta, -vy), or FLUID ghost rows; they are loaded like any row.
 #include <cstdlib>
 #include <type_traits>
-#include <cuda.h>      // CUtensorMap (types only; the encoder is fetched through the runtime, no -lcuda)
 #include "vlasov_internal.cuh"
+#include "tma.cuh"
 
 namespace vl {
 
@@ -36,30 +36,6 @@ struct XYParams {
     double finf;
     int bc_lo, bc_hi;
 };
-
-// ---- mbarriers and tiled TMA: rows land in shared memory without passing registers ----
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// 2D tiled TMA: box {PC cells, nx spatial cells} of row `c1 / nx` lands dense in shared memory as [x][PC]
-__device__ __forceinline__ void tma_g2s_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-                 ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(bar) : "memory");
-}
 
 struct Weights {
     double w0, w1, w2;     // alpha, alpha (1-a)(2-a)/6, alpha (1-a)(1+a)/6 of eq. (46): uniform along a line
@@ -351,27 +327,6 @@ static void launch_xy_t(const CUtensorMap& tm, const XYParams& P, int xfirst, di
     }
 }
 
-// Tensor map of one species' f seen as a matrix [ny_g * nx spatial cells][S velocity cells] of fp64, box
-// {pc cells, nx spatial cells}.  The encoder is a driver entry point fetched through the runtime.
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-static bool make_row_map(CUtensorMap* tm, const double* base, long S, long ncell, int pc, int nx) {
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || !p) return false;
-        fn = (EncodeTiledFn)p;
-    }
-    const cuuint64_t dims[2] = {(cuuint64_t)S, (cuuint64_t)ncell};
-    const cuuint64_t strides[1] = {(cuuint64_t)S * 8};
-    const cuuint32_t box[2] = {(cuuint32_t)pc, (cuuint32_t)nx};
-    const cuuint32_t estr[2] = {1, 1};
-    return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 // Shared memory of the fused kernel: barriers, weight table, NS raw rows (+ 2 y-swept rows), each row made of
 // 128-byte aligned pieces.
 static size_t xy_smem_bytes(const Geom& G, const Species& s, int C, int xfirst) {
@@ -434,7 +389,7 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     P.PC = C < s.nv[2] ? C : s.nv[2];
     const size_t smem = xy_smem_bytes(G, s, C, xfirst);
     CUtensorMap tm;
-    if (!make_row_map(&tm, src, s.nvtot, (long)G.nyg * G.nx, P.PC, G.nx)) return VLASOV_ECUDA;
+    if (!make_tensor_map_2d(&tm, src, s.nvtot, (long)G.nyg * G.nx, P.PC, G.nx)) return VLASOV_ECUDA;
     dim3 grid((unsigned)(s.nvtot / C));
     const int threads = nblk * C;
     const int lim = G.limiter ? 1 : 0;

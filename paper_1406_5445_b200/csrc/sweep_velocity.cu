@@ -12,6 +12,7 @@
 // second shared array, then every cell is updated by eq. (38).  vx: tile = all i_vx x 128 contiguous
 // (i_vy,i_vz) cells.  vy+vz fused: tile = a few contiguous i_vx planes.  In place on f.
 #include "vlasov_internal.cuh"
+#include "tma.cuh"
 
 namespace vl {
 
@@ -373,6 +374,63 @@ __global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams
 }
 
 // ------------------------------------------------------------------------------------------------
+// a4 with the tiles prefetched: the same walk, but the tile of the NEXT two visits of this CTA is already on
+// its way when a tile is worked on (2D tiled TMA, box {128 columns, CN rows}, one instruction per tile, two
+// buffers + mbarriers).  The plain kernel above spends about 40 % of its stall samples waiting for its own
+// global loads (profiles/).  CN^3 blocks with CN^2 a multiple of 128; not for the ghost fill (its tiles read
+// another cell and are scaled).  Shared memory, in rows of 128 doubles:
+//   [V_PAD zero rows][CN rows, buffer 0][V_PAD zero rows][CN rows, buffer 1][V_PAD zero rows][2 mbarriers]
+// ------------------------------------------------------------------------------------------------
+template <int LIM, int CN>
+__global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
+    extern __shared__ __align__(128) double sm[];
+    constexpr int CT = 128, N = CN, plane = CN * CN, ntile = plane / CT, nsegx = CN / 8, seglen = 8;
+    constexpr int ROWS = 3 * V_PAD + 2 * CN;
+    // only the three pad strips are ever written by threads (zeros, once); the buffers belong to the TMA unit
+    for (int e = threadIdx.x; e < V_PAD * CT; e += V_THREADS) {
+        sm[e] = 0.0; sm[(V_PAD + CN) * CT + e] = 0.0; sm[(2 * V_PAD + 2 * CN) * CT + e] = 0.0;
+    }
+    const unsigned bar0 = smem_addr(sm + ROWS * CT);
+    const unsigned sbuf0 = smem_addr(sm + V_PAD * CT);
+    constexpr unsigned BUFSTEP = (unsigned)(CN + V_PAD) * CT * 8;
+    if (threadIdx.x == 0) { mbar_init(bar0, 1); mbar_init(bar0 + 8, 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    auto issue = [&](int tile, int b) {            // thread 0 only
+        const int cell = P.cell0 + tile / ntile;
+        mbar_expect_tx(bar0 + 8 * b, (unsigned)CN * CT * 8);
+        tma_g2s_2d(sbuf0 + b * BUFSTEP, &tmap, (tile % ntile) * CT, cell * CN, bar0 + 8 * b);
+    };
+    if (threadIdx.x == 0) {
+        if ((int)blockIdx.x < P.ntot) issue(blockIdx.x, 0);
+        if ((int)(blockIdx.x + gridDim.x) < P.ntot) issue(blockIdx.x + gridDim.x, 1);
+    }
+    int it = 0;
+    for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x, ++it) {
+        const int b = it & 1;
+        const int cell = P.cell0 + tile / ntile;
+        const int c0 = (tile % ntile) * CT;
+        const double* T = P.table + (long)cell * TAB;
+        const double t0 = T[0], t1 = T[1], t2 = T[2], t3 = T[3], finf = T[12];
+        double* fb = P.f + (long)cell * P.S + c0;
+        const double* A = sm + (V_PAD + b * (CN + V_PAD)) * CT;
+        mbar_wait(bar0 + 8 * b, (it >> 1) & 1);
+#pragma unroll
+        for (int wi = threadIdx.x; wi < CT * nsegx; wi += V_THREADS) {
+            const int seg = wi / CT, c = wi - seg * CT;
+            const int col = c0 + c;
+            const int k1 = col / CN, k2 = col - k1 * CN;
+            const double s0 = t0 + t2 * k1 + t3 * k2;
+            const int a = seg * seglen;
+            OutGlobal o{fb + c + (long)a * plane, (long)plane};
+            march_cells<LIM, 1>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);
+        }
+        __syncthreads();                           // everybody is done reading buffer b: refill it
+        if (threadIdx.x == 0 && tile + 2 * (int)gridDim.x < P.ntot) issue(tile + 2 * gridDim.x, b);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // a5 + a6: vy sweep then vz sweep on a tile of PT contiguous i_vx planes.  Shared layout of a buffer:
 // cell (p, y, z) at OFF + p PS + y RS + z with RS = N2 + V_PAD (odd: threads that march neighbouring z
 // lines hit distinct banks), PS = (N1 + V_PAD) RS, OFF = V_PAD RS + V_PAD; everything that is not a cell is zero and
@@ -495,7 +553,7 @@ static int resident_ctas(K kernel, size_t smem, int& cache, size_t& cache_smem) 
     return cache;
 }
 
-int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows) {
+int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost) {
     if (nrows <= 0) return VLASOV_OK;
     VParams P;
     P.f = f; P.table = c->table; P.S = s.nvtot;
@@ -521,9 +579,24 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 16) k = lim ? vsweep_x_kernel<1, 16> : vsweep_x_kernel<0, 16>;
         if (spec == 32) k = lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>;
         const int cube32 = spec ? 1 : 0;
-        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim + 2 * cube32], g_occ_x_smem[lim + 2 * cube32]));
-        Launch L(c, K_VSWEEP_X);
-        k<<<grid, V_THREADS, smem, c->stream>>>(P);
+        if (spec && !ghost) {
+            // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]
+            CUtensorMap tm;
+            if (!make_tensor_map_2d(&tm, f, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, spec)) return VLASOV_ECUDA;
+            void (*kt)(CUtensorMap, VParams) = lim ? vsweep_x_tma_kernel<1, 32> : vsweep_x_tma_kernel<0, 32>;
+            if (spec == 16) kt = lim ? vsweep_x_tma_kernel<1, 16> : vsweep_x_tma_kernel<0, 16>;
+            const size_t smem_t = (size_t)(3 * V_PAD + 2 * spec) * 128 * 8 + 16;
+            static int occ_t[4] = {0, 0, 0, 0};
+            static size_t occ_t_smem[4] = {0, 0, 0, 0};
+            const int gi = lim + (spec == 16 ? 2 : 0);
+            const int grid = min(P.ntot, resident_ctas(kt, smem_t, occ_t[gi], occ_t_smem[gi]));
+            Launch L(c, K_VSWEEP_X);
+            kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);
+        } else {
+            const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim + 2 * cube32], g_occ_x_smem[lim + 2 * cube32]));
+            Launch L(c, K_VSWEEP_X);
+            k<<<grid, V_THREADS, smem, c->stream>>>(P);
+        }
     }
     {
         const size_t rs = s.nv[2] + V_PAD, ps = (s.nv[1] + V_PAD) * rs, off = V_PAD * rs + V_PAD;

@@ -96,7 +96,8 @@ bool fused_xy_applicable(const vlasov_ctx* c, const Species& s, double dts);
 int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int xfirst);
 // Lorentz table (a3) and velocity sweeps (a4-a6), in place on f, rows [row0, row0+nrows)
 int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const double* B, double dt);
-int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows);
+// ghost: the launch is a ghost fill (tiles read the edge cell T[16] and are scaled by T[15])
+int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost = false);
 // moments (a9): out[11][nyg*nx] (10 moments + max f) of rows [row0,row0+nrows) of f
 int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out, int row0, int nrows);
 // ghost fill (a0) of one side
