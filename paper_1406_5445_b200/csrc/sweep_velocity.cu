@@ -535,6 +535,105 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// a5 + a6 with the tile loaded by 2D tiled TMA (one box {CN, CN} per plane) into a dense staging buffer with zero
+// pad rows between the planes: the vy sweep reads it directly (lanes run along z: any pitch is conflict-free) and
+// writes the padded, odd-pitch buffer Bf; as soon as the vy sweep is done the staging buffer is free and the NEXT
+// tile's load is issued, landing while the vz sweep (Bf -> A) and the store (A -> global) run.  No load instruction,
+// no exposed load latency, two block barriers per tile instead of four, and still 3 CTAs per SM for 32x32 planes.
+//   shared: [staging: 8 + ct (CN + 8) rows of CN][Bf][A][mbarrier]
+// ------------------------------------------------------------------------------------------------
+template <int LIM, int CN>
+__global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
+    extern __shared__ __align__(128) double sm[];
+    constexpr int N1 = CN, N2 = CN, plane = CN * CN;
+    constexpr int ct = (8 * V_THREADS) / plane > 0 ? (8 * V_THREADS) / plane : 1;
+    constexpr int nseg = (CN + 7) / 8, seglen = (CN + nseg - 1) / nseg;
+    constexpr int RS = N2 + V_PAD, PS = (N1 + V_PAD) * RS, OFF = V_PAD * RS + V_PAD;
+    constexpr int BUF = (OFF + ct * PS + 1) & ~1;
+    constexpr int SPAD = 8;                                      // pad rows of the staging buffer: >= V_PAD, and 8 rows of
+                                                                 // any even N2 keep every TMA box 128-byte aligned
+    constexpr int SROWS = SPAD + ct * (N1 + SPAD);               // staging rows of N2 doubles
+    constexpr int STG = (SROWS * N2 + 15) & ~15;                 // keeps Bf 128-byte aligned
+    if (P.ct != ct || P.nseg != nseg || P.nseg2 != nseg || P.nv1 != CN || P.nv2 != CN) return;
+    double* St = sm;
+    double* Bf = sm + STG;
+    double* A = Bf + BUF;
+    const unsigned bar = smem_addr(A + BUF);
+    // zero: the staging pad rows (never written again), Bf and A entirely (their cells are overwritten per tile)
+    for (int e = threadIdx.x; e < SPAD * N2; e += V_THREADS) {
+        St[e] = 0.0;
+#pragma unroll
+        for (int p = 0; p < ct; ++p) St[(SPAD + p * (N1 + SPAD) + N1) * N2 + e] = 0.0;
+    }
+    for (int e = threadIdx.x; e < 2 * BUF; e += V_THREADS) Bf[e] = 0.0;
+    if (threadIdx.x == 0) mbar_init(bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    const unsigned sSt = smem_addr(St), sA = smem_addr(A);
+    auto issue = [&](int tile) {                   // thread 0 only: ct boxes, one per plane
+        const int cell = P.cell0 + tile / P.ntile;
+        const int p0 = (tile % P.ntile) * ct;
+        mbar_expect_tx(bar, (unsigned)ct * plane * 8);
+#pragma unroll
+        for (int p = 0; p < ct; ++p)
+            tma_g2s_2d(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2) * 8, &tmap, 0, (cell * P.nv0 + p0 + p) * N1, bar);
+    };
+    if (threadIdx.x == 0 && (int)blockIdx.x < P.ntot) issue(blockIdx.x);
+    // staging map of the store loop (as in the plain kernel)
+    const int z_init = threadIdx.x % N2, row_init = threadIdx.x / N2;
+    const int y_init = row_init % N1;
+    const unsigned so_init = OFF + (row_init / N1) * PS + y_init * RS + z_init;
+    constexpr int dz = V_THREADS % N2, drow = V_THREADS / N2, dy = drow % N1;
+    constexpr unsigned dso = dz + dy * RS + (drow / N1) * PS;
+    constexpr int ncellt = ct * plane;
+    int it = 0;
+    for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x, ++it) {
+        const int cell = P.cell0 + tile / P.ntile;
+        const int p0 = (tile % P.ntile) * ct;
+        double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
+        const double* T = P.table + (long)cell * TAB;
+        const double ty0 = T[4], ty1 = T[5], ty2 = T[6], ty3 = T[7], finfy = T[13];
+        const double tz0 = T[8], tz1 = T[9], tz2 = T[10], tz3 = T[11], finfz = T[14];
+        mbar_wait(bar, it & 1);
+        {   // vy: line along i_vy (stride N2 in the staging buffer); transverse (plane, i_vz); threads run along z
+            constexpr int nl = ct * N2;
+            for (int wi = threadIdx.x; wi < nl * nseg; wi += V_THREADS) {
+                const int seg = wi / nl, l = wi - seg * nl;
+                const int p = l / N2, z = l - p * N2;
+                const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
+                const int a = seg * seglen, b = min(a + seglen, N1);
+                OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
+                march_cells<LIM, 1>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+            }
+        }
+        __syncthreads();                           // vy done: Bf complete, staging buffer free
+        if (threadIdx.x == 0 && tile + (int)gridDim.x < P.ntot) issue(tile + gridDim.x);
+        {   // vz: contiguous lines of Bf; transverse (plane, i_vy); threads run along y (pitch RS, odd)
+            constexpr int nl = ct * N1;
+            for (int wi = threadIdx.x; wi < nl * nseg; wi += V_THREADS) {
+                const int seg = wi / nl, l = wi - seg * nl;
+                const int p = l / N1, y = l - p * N1;
+                const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
+                const int a = seg * seglen, b = min(a + seglen, N2);
+                OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
+                march_cells<LIM, 1>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
+            }
+        }
+        __syncthreads();                           // vz done: A complete
+        {   // A -> global (the next tile's vz sweep writes A only after the next barrier)
+            int z = z_init, y = y_init;
+            unsigned so = so_init;
+            for (int e = threadIdx.x; e < ncellt; e += V_THREADS) {
+                __stcs(fb + e, lds(sA + so * 8));
+                z += dz; y += dy; so += dso;
+                if (z >= N2) { z -= N2; so += RS - N2; ++y; }
+                if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+            }
+        }
+    }
+}
+
 static int g_occ_x[4] = {0, 0, 0, 0}, g_occ_yz[4] = {0, 0, 0, 0};
 static size_t g_occ_x_smem[4] = {0, 0, 0, 0}, g_occ_yz_smem[4] = {0, 0, 0, 0};
 constexpr size_t V_SMEM_MAX = 200 * 1024;
@@ -623,9 +722,30 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
         if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
         const int sq32 = spec ? 1 : 0;
-        const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim + 2 * sq32], g_occ_yz_smem[lim + 2 * sq32]));
-        Launch L(c, K_VSWEEP_YZ);
-        k<<<grid, V_THREADS, smem, c->stream>>>(P);
+        if (spec) {
+            // TMA-staged variant: f as a matrix [cells * nv0 * nv1][nv2], one box {nv2, nv1} per plane
+            CUtensorMap tm;
+            if (!make_tensor_map_2d(&tm, f, s.nv[2], (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1], s.nv[2], s.nv[1])) return VLASOV_ECUDA;
+            void (*kt)(CUtensorMap, VParams) = lim ? vsweep_yz_tma_kernel<1, 32> : vsweep_yz_tma_kernel<0, 32>;
+            if (spec == 16) kt = lim ? vsweep_yz_tma_kernel<1, 16> : vsweep_yz_tma_kernel<0, 16>;
+            if (spec == 24) kt = lim ? vsweep_yz_tma_kernel<1, 24> : vsweep_yz_tma_kernel<0, 24>;
+            if (spec == 40) kt = lim ? vsweep_yz_tma_kernel<1, 40> : vsweep_yz_tma_kernel<0, 40>;
+            if (spec == 48) kt = lim ? vsweep_yz_tma_kernel<1, 48> : vsweep_yz_tma_kernel<0, 48>;
+            const size_t srows = 8 + (size_t)pt * (s.nv[1] + 8);
+            const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
+            const size_t smem_t = (stg + 2 * buf) * 8 + 16;
+            if (smem_t > V_SMEM_MAX) return VLASOV_EINVAL;
+            static int occ_t[16] = {0};
+            static size_t occ_t_smem[16] = {0};
+            const int gi = lim + 2 * (spec / 8);
+            const int grid = min(P.ntot, resident_ctas(kt, smem_t, occ_t[gi], occ_t_smem[gi]));
+            Launch L(c, K_VSWEEP_YZ);
+            kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);
+        } else {
+            const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim + 2 * sq32], g_occ_yz_smem[lim + 2 * sq32]));
+            Launch L(c, K_VSWEEP_YZ);
+            k<<<grid, V_THREADS, smem, c->stream>>>(P);
+        }
     }
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
