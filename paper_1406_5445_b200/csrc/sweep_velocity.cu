@@ -722,7 +722,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
         if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
         const int sq32 = spec ? 1 : 0;
-        if (spec) {
+        if (spec && spec != 48) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
             // TMA-staged variant: f as a matrix [cells * nv0 * nv1][nv2], one box {nv2, nv1} per plane
             CUtensorMap tm;
             if (!make_tensor_map_2d(&tm, f, s.nv[2], (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1], s.nv[2], s.nv[1])) return VLASOV_ECUDA;
@@ -730,7 +730,6 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (spec == 16) kt = lim ? vsweep_yz_tma_kernel<1, 16> : vsweep_yz_tma_kernel<0, 16>;
             if (spec == 24) kt = lim ? vsweep_yz_tma_kernel<1, 24> : vsweep_yz_tma_kernel<0, 24>;
             if (spec == 40) kt = lim ? vsweep_yz_tma_kernel<1, 40> : vsweep_yz_tma_kernel<0, 40>;
-            if (spec == 48) kt = lim ? vsweep_yz_tma_kernel<1, 48> : vsweep_yz_tma_kernel<0, 48>;
             const size_t srows = 8 + (size_t)pt * (s.nv[1] + 8);
             const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
             const size_t smem_t = (stg + 2 * buf) * 8 + 16;
