@@ -185,7 +185,7 @@ __device__ __forceinline__ int need_bits(double f0, double dp, double dm, double
 // (eq. 47 = eq. 46 on the mirrored line), and face m of the walk takes (q[m], q[m+1], q[m+2]).  About a
 // quarter of the instructions of the general walk below.
 //   walk position i <-> cell a-2+i (sigma >= 0) | a+SEG+1-i (sigma < 0);  face m <-> face a+m | a+SEG-m.
-template <int SEG, int LIM, class Out>
+template <int SEG, int LIM, int FULL, class Out>
 __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
                                                 double s1, double finf, Out out) {
     const bool pos = !(sig_a < 0.0 || sig_b < 0.0);      // the caller made sure the two do not disagree
@@ -206,7 +206,7 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
 #pragma unroll
     for (int m = 0; m <= SEG; ++m) {
         double sp, sm;
-        slopes_fast<LIM>(q[m], q[m + 1], q[m + 2], finf, sp, sm);     // all lanes sit on the same face: one vote per face
+        slopes_fast<LIM, FULL>(q[m], q[m + 1], q[m + 2], finf, sp, sm);     // all lanes sit on the same face: one vote per face
         const double bq = fabs(sig);
         const double b2 = bq * bq;
         const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
@@ -225,7 +225,7 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
 // in the direction of the flow, q[i] <-> cell a-3-n0+i (sigma >= 0) | a+SEG+n0+2-i (sigma < 0), and face m takes
 // (q[m+1-e], q[m+2-e], q[m+3-e]) with e = floor|sigma_m| - n0 in {0, 1}.  Whole cells of eqs. (46)/(47) and the
 // cell being updated come from shared memory.
-template <int SEG, int LIM, class Out>
+template <int SEG, int LIM, int FULL, class Out>
 __device__ __forceinline__ void march_seg_window(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
                                                  double s1, double finf, Out out, int n0, bool pos) {
     const double M = 6755399441055744.0;
@@ -255,7 +255,7 @@ __device__ __forceinline__ void march_seg_window(unsigned L, int st8, int N, int
         const double fm = e ? q[m] : q[m + 1];
         const double fp = e ? q[m + 2] : q[m + 3];
         double sp, sm;
-        slopes_fast<LIM>(fm, f0, fp, finf, sp, sm);
+        slopes_fast<LIM, FULL>(fm, f0, fp, finf, sp, sm);
         double sum = 0.0;
         if (n > 0) {                                 // whole cells k-n .. k-1 (sigma >= 0) | k .. k+n-1 (sigma < 0), ascending
             unsigned as_ = pos ? wh - n * st8 : wh;
@@ -290,10 +290,12 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
         const int n0 = min(na, nb);
         const bool one_way = !(sig * sig_b < 0.0) && fabs(sig) < 64.0 && fabs(sig_b) < 64.0;
         const bool window = one_way && abs(na - nb) <= 1 && n0 <= (pos ? a : N - a - SEG) + V_PAD - 3;
-        const unsigned mask = __activemask();
+        // FAST == 2: every lane of the warp is here (work items are a multiple of the block size)
+        constexpr int FULL = FAST == 2 ? 1 : 0;
+        const unsigned mask = FULL ? 0xffffffffu : __activemask();
         if (__all_sync(mask, window)) {
-            if (__all_sync(mask, (na | nb) == 0)) march_seg_small<SEG, LIM>(L, st8, N, a, sig, sig_b, s1, finf, out);
-            else march_seg_window<SEG, LIM>(L, st8, N, a, sig, sig_b, s1, finf, out, n0, pos);
+            if (__all_sync(mask, (na | nb) == 0)) march_seg_small<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            else march_seg_window<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out, n0, pos);
             return;
         }
     }
@@ -423,7 +425,7 @@ __global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid
             const double s0 = t0 + t2 * k1 + t3 * k2;
             const int a = seg * seglen;
             OutGlobal o{fb + c + (long)a * plane, (long)plane};
-            march_cells<LIM, 1>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);
+            march_cells<LIM, 2>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);     // 512 items, 256 threads: full warps
         }
         __syncthreads();                           // everybody is done reading buffer b: refill it
         if (threadIdx.x == 0 && tile + 2 * (int)gridDim.x < P.ntot) issue(tile + 2 * gridDim.x, b);
@@ -555,6 +557,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
                                                                  // any even N2 keep every TMA box 128-byte aligned
     constexpr int SROWS = SPAD + ct * (N1 + SPAD);               // staging rows of N2 doubles
     constexpr int STG = (SROWS * N2 + 15) & ~15;                 // keeps Bf 128-byte aligned
+    constexpr int FW = (ct * CN * nseg) % V_THREADS == 0 ? 2 : 1; // 2: the work items fill whole warps (march_cells)
     if (P.ct != ct || P.nseg != nseg || P.nseg2 != nseg || P.nv1 != CN || P.nv2 != CN) return;
     double* St = sm;
     double* Bf = sm + STG;
@@ -604,7 +607,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
                 const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
                 const int a = seg * seglen, b = min(a + seglen, N1);
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM, 1>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+                march_cells<LIM, FW>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
@@ -617,7 +620,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
                 const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
                 const int a = seg * seglen, b = min(a + seglen, N2);
                 OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
-                march_cells<LIM, 1>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
+                march_cells<LIM, FW>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
             }
         }
         __syncthreads();                           // vz done: A complete

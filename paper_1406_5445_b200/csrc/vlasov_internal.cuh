@@ -164,7 +164,8 @@ __device__ __forceinline__ double relu_bits(double x) {
 //     hi(|d|) < min(hi(2 f0), hi(2 (f_inf - f0)))   ==>   |d| < min(2 f0, 2 (f_inf - f0))   ==>   eps = 1.
 // The test is conservative (ties and negative bounds fall through to the exact clamps); hi(2 x) is
 // hi(x) + 2^20 (exponent + 1; the denormal corner only ever errs by < 1e-307).
-template <int LIM>
+// FULL: the caller guarantees that all 32 lanes of the warp make this call (saves the active-mask bookkeeping).
+template <int LIM, int FULL = 0>
 __device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, double finf, double& sp, double& sm) {
     const double dp = fp - f0, dm = f0 - fm;
     sp = dp; sm = dm;
@@ -173,7 +174,7 @@ __device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, dou
         const int hf = __double2hiint(f0) + 0x00100000, hg = __double2hiint(g) + 0x00100000;
         const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
         const int hmax = max(hp, hm);
-        const unsigned mask = __activemask();
+        const unsigned mask = FULL ? 0xffffffffu : __activemask();
         if (__any_sync(mask, hmax >= min(hf, hg))) {
             const double hiA = relu_bits(f0 + f0);
             if (!__any_sync(mask, hmax >= hg)) {
