@@ -681,7 +681,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 16) k = lim ? vsweep_x_kernel<1, 16> : vsweep_x_kernel<0, 16>;
         if (spec == 32) k = lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>;
         const int cube32 = spec ? 1 : 0;
-        if (spec && !ghost) {
+        if (spec && !ghost && (long)c->G.nyg * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
             // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]
             CUtensorMap tm;
             if (!make_tensor_map_2d(&tm, f, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, spec)) return VLASOV_ECUDA;
@@ -725,7 +725,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
         if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
         const int sq32 = spec ? 1 : 0;
-        if (spec && spec != 48) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
+        if (spec && spec != 48 && (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1] < 2147483647L) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
             // TMA-staged variant: f as a matrix [cells * nv0 * nv1][nv2], one box {nv2, nv1} per plane
             CUtensorMap tm;
             if (!make_tensor_map_2d(&tm, f, s.nv[2], (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1], s.nv[2], s.nv[1])) return VLASOV_ECUDA;
