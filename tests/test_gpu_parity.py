@@ -143,14 +143,16 @@ def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
     assert rel_l2(fg[0], fu[0]) <= TOL1
 
 
-@pytest.mark.parametrize("nv", [(12, 10, 14), (8, 16, 32), (32, 32, 32)])
+@pytest.mark.parametrize("nv", [(12, 10, 14), (8, 16, 32), (32, 32, 32), (24, 24, 24), (4, 40, 40), (6, 48, 48), (16, 16, 16)])
 @pytest.mark.parametrize("fields_yee", [0, 1])
 def test_velocity_step_multicell_shifts(gpu, orc, fields_yee, nv):
     """a3-a6: strong fields give sign-changing shifts of several cells; Yee gather vs cell-centred.  (12,10,14):
     ragged segments, the general face walk; (8,16,32) and 32^3: 8-cell segments, the register-window walks (and for
-    32^3 the compile-time-shape kernels) wherever floor|sigma| is steady enough along the segment."""
+    32^3 the compile-time-shape, TMA-staged kernels) wherever floor|sigma| is steady enough along the segment; the
+    other shapes are the remaining compile-time-shape kernels (16, 24, 40: TMA-staged vy+vz; 48: plain; 16^3: TMA vx)."""
     rng = np.random.default_rng(2)
-    w = random_workload(rng, nx=5 if nv[0] < 32 else 3, ny=4 if nv[0] < 32 else 2, nv=nv, bc=inputs.BC_REFLECT,
+    big = nv[0] * nv[1] * nv[2] > 8000
+    w = random_workload(rng, nx=3 if big else 5, ny=2 if big else 4, nv=nv, bc=inputs.BC_REFLECT,
                         fields_yee=fields_yee)
     f0 = [smooth_random_f(rng, w, 0)]
     E = 6.0 * rng.standard_normal((3, w.ny_g, w.nx))
