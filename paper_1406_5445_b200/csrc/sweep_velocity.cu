@@ -155,9 +155,9 @@ __device__ __forceinline__ double face_flux_pad(unsigned L, int st8, int N, int 
     return __hiloint2double(__double2hiint(phi) ^ (sg & 0x80000000), __double2loint(phi));
 }
 
-// Zero cells on either side of every line of the vy/vz tile (f = 0 outside the box, R7): 3 would do for the
-// general walk (foot clamped to [-2, N+1]); the register-window walk reads up to V_PAD - 3 cells further out.
-constexpr int V_PAD = 7;
+// Zero cells on either side of every line of a tile (f = 0 outside the box, R7): the general walk clamps the foot to
+// [-2, N+1] and reads its two neighbours, the register-window walk reads cells -2 .. N+1.
+constexpr int V_PAD = 3;
 
 struct OutShared {       // cells of a line in shared memory: cell0 = byte address of cell a
     unsigned a; int st8;
@@ -219,61 +219,6 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
     }
 }
 
-// The same walk for shifts of any size, as long as along the segment floor|sigma| takes at most two neighbouring
-// values n0, n0 + 1 and sigma keeps its sign (sigma is affine in the face index and varies by a small fraction
-// of a cell over 8 faces, so this is the rule): the window is read relative to the foot cells, SEG + 4 cells
-// in the direction of the flow, q[i] <-> cell a-3-n0+i (sigma >= 0) | a+SEG+n0+2-i (sigma < 0), and face m takes
-// (q[m+1-e], q[m+2-e], q[m+3-e]) with e = floor|sigma_m| - n0 in {0, 1}.  Whole cells of eqs. (46)/(47) and the
-// cell being updated come from shared memory.
-template <int SEG, int LIM, int FULL, class Out>
-__device__ __forceinline__ void march_seg_window(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
-                                                 double s1, double finf, Out out, int n0, bool pos) {
-    const double M = 6755399441055744.0;
-    const int dir = pos ? 1 : -1;
-    const int ust8 = pos ? st8 : -st8;
-    unsigned addr = L + (pos ? a - 3 - n0 : a + SEG + n0 + 2) * st8;
-    double q[SEG + 4];
-#pragma unroll
-    for (int i = 0; i < SEG + 4; ++i) { q[i] = lds(addr); addr += ust8; }
-    const bool zero_first = pos ? a == 0 : a + SEG == N;
-    const bool zero_last = pos ? a + SEG == N : a == 0;
-    double sig = pos ? sig_a : sig_b;
-    const double ds = pos ? s1 : -s1;
-    unsigned own = L + (pos ? a : a + SEG - 1) * st8;              // cell between walk faces 0 and 1
-    unsigned wh = L + (pos ? a : a + SEG) * st8;                   // face of walk step 0, as a cell address
-    if (!pos) { out.skip(SEG - 1); }
-    out.step(dir);
-    double Gp = 0.0;
-#pragma unroll
-    for (int m = 0; m <= SEG; ++m) {
-        const double as = fabs(sig);
-        const double r = __dadd_rd(as, M);
-        const int n = __double2loint(r);
-        const double bq = as - (r - M);
-        const bool e = n != n0;
-        const double f0 = e ? q[m + 1] : q[m + 2];
-        const double fm = e ? q[m] : q[m + 1];
-        const double fp = e ? q[m + 2] : q[m + 3];
-        double sp, sm;
-        slopes_fast<LIM, FULL>(fm, f0, fp, finf, sp, sm);
-        double sum = 0.0;
-        if (n > 0) {                                 // whole cells k-n .. k-1 (sigma >= 0) | k .. k+n-1 (sigma < 0), ascending
-            unsigned as_ = pos ? wh - n * st8 : wh;
-#pragma unroll 1
-            for (int t = 0; t < n; ++t) { sum += lds(as_); as_ += st8; }
-        }
-        const double b2 = bq * bq;
-        const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
-        const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
-        double G = fma(bq, fma(c1, sp, fma(c2, sm, f0)), sum);
-        if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
-        if (m > 0) { out.put(lds(own) + (Gp - G)); own += ust8; }
-        Gp = G;
-        sig += ds;
-        wh += ust8;
-    }
-}
-
 // One thread remaps cells [a, b) of one line: flux per face, eq. (38) per cell.  sigma of face k is
 // s0 + s1 k (accumulated).  out.put(value) stores the new average of the next cell (a, a+1, ...).
 template <int LIM, int FAST, class Out>
@@ -282,20 +227,14 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
     double sig = fma(s1, (double)a, s0);
     constexpr int SEG = 8;
     if (FAST && b - a == SEG) {
-        // sigma is affine along the line: what holds for floor|sigma| and the sign at both end faces holds between
-        const double Mg = 6755399441055744.0;
+        // sigma is affine along the line: |sigma| < 1 and one sign at both end faces hold on every face between.
+        // (A register-window walk for multi-cell shifts was built and measured: its whole-cell sum loops cost what
+        // the general walk's addressing costs -- DESIGN.md section 11.)
         const double sig_b = fma(s1, (double)b, s0);
-        const int na = __double2loint(__dadd_rd(fabs(sig), Mg)), nb = __double2loint(__dadd_rd(fabs(sig_b), Mg));
-        const bool pos = !(sig < 0.0 || sig_b < 0.0);
-        const int n0 = min(na, nb);
-        const bool one_way = !(sig * sig_b < 0.0) && fabs(sig) < 64.0 && fabs(sig_b) < 64.0;
-        const bool window = one_way && abs(na - nb) <= 1 && n0 <= (pos ? a : N - a - SEG) + V_PAD - 3;
-        // FAST == 2: every lane of the warp is here (work items are a multiple of the block size)
-        constexpr int FULL = FAST == 2 ? 1 : 0;
-        const unsigned mask = FULL ? 0xffffffffu : __activemask();
-        if (__all_sync(mask, window)) {
-            if (__all_sync(mask, (na | nb) == 0)) march_seg_small<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out);
-            else march_seg_window<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out, n0, pos);
+        const bool small = fabs(sig) < 1.0 && fabs(sig_b) < 1.0 && !(sig * sig_b < 0.0);
+        constexpr int FULL = FAST == 2 ? 1 : 0;        // FAST == 2: every lane of the warp is here
+        if (__all_sync(FULL ? 0xffffffffu : __activemask(), small)) {
+            march_seg_small<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out);
             return;
         }
     }
