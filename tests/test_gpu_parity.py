@@ -147,8 +147,8 @@ def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
 @pytest.mark.parametrize("fields_yee", [0, 1])
 def test_velocity_step_multicell_shifts(gpu, orc, fields_yee, nv):
     """a3-a6: strong fields give sign-changing shifts of several cells; Yee gather vs cell-centred.  (12,10,14):
-    ragged segments, the general face walk; (8,16,32) and 32^3: 8-cell segments, the register-window walks (and for
-    32^3 the compile-time-shape, TMA-staged kernels) wherever floor|sigma| is steady enough along the segment; the
+    ragged segments, the general face walk; (8,16,32) and 32^3: 8-cell segments, the register-window walk wherever a
+    whole warp has |sigma| < 1 (and for 32^3 the compile-time-shape, TMA-staged kernels); the
     other shapes are the remaining compile-time-shape kernels (16, 24, 40: TMA-staged vy+vz; 48: plain; 16^3: TMA vx)."""
     rng = np.random.default_rng(2)
     big = nv[0] * nv[1] * nv[2] > 8000
