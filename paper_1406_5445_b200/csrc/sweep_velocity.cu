@@ -241,7 +241,7 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
     double phi_lo = a > 0 ? face_flux_pad<LIM>(L, st8, N, a, sig, finf) : 0.0;
     unsigned ci = L + a * st8;
     const int bi = b < N ? b : N - 1;                // faces a+1 .. bi are interior
-#pragma unroll 2
+#pragma unroll 4
     for (int k = a + 1; k <= bi; ++k) {
         sig += s1;
         const double phi_hi = face_flux_pad<LIM>(L, st8, N, k, sig, finf);
