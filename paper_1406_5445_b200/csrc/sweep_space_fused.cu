@@ -149,15 +149,17 @@ __device__ __forceinline__ int virtual_row(const XYParams& P, int r, bool& mirro
 // rows ahead of the row being worked on.
 constexpr int XY_NS = 5;
 
-// SP > 0: nx = SP spatial cells per row, 32^3 velocity cells, the launcher's chunk for that (C = PC = 2048 / SP):
-// every stride of the kernel is a compile-time constant.  SP = 0: any shape, at run time.
-template <int XB, int LIM, int XFIRST, int SP>
+constexpr int xy_default_chunk(int sp) { return sp > 0 ? 2048 / (sp > 0 ? sp : 1) : 0; }
+
+// SP > 0: nx = SP spatial cells per row, NV^3 velocity cells, KC = the launcher's chunk for that shape (one piece:
+// C = PC = KC): every stride of the kernel is a compile-time constant.  SP = 0: any shape, at run time.
+template <int XB, int LIM, int XFIRST, int SP, int NV = 32, int KC = xy_default_chunk(SP)>
 __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant__ CUtensorMap tmap, XYParams P) {
     extern __shared__ __align__(128) unsigned char smraw[];
-    constexpr int KC = SP ? 2048 / SP : 0;
-    if (SP && (P.nx != SP || P.C != KC || P.PC != KC || P.nv1 != 32 || P.nv2 != 32 || P.S != 32768)) return;
-    const int nx = SP ? SP : P.nx, nv1 = SP ? 32 : P.nv1, nv2 = SP ? 32 : P.nv2;
-    const long S = SP ? 32768 : P.S, row_stride = SP ? (long)SP * 32768 : P.row_stride;
+    constexpr long KS = (long)NV * NV * NV;
+    if (SP && (P.nx != SP || P.C != KC || P.PC != KC || P.nv1 != NV || P.nv2 != NV || P.S != KS)) return;
+    const int nx = SP ? SP : P.nx, nv1 = SP ? NV : P.nv1, nv2 = SP ? NV : P.nv2;
+    const long S = SP ? KS : P.S, row_stride = SP ? (long)SP * KS : P.row_stride;
     const int C = SP ? KC : P.C, C8 = C * 8;
     const int c = threadIdx.x % C, blk = threadIdx.x / C;
     const int ix0 = blk * XB;
@@ -315,15 +317,15 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
     }
 }
 
-template <int XB, int LIM, int SP>
+template <int XB, int LIM, int SP, int NV = 32, int KC = xy_default_chunk(SP)>
 static void launch_xy_t(const CUtensorMap& tm, const XYParams& P, int xfirst, dim3 grid, int threads, size_t smem,
                         cudaStream_t st) {
     if (xfirst) {
-        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 1, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        sweep_xy_kernel<XB, LIM, 1, SP><<<grid, threads, smem, st>>>(tm, P);
+        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 1, SP, NV, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        sweep_xy_kernel<XB, LIM, 1, SP, NV, KC><<<grid, threads, smem, st>>>(tm, P);
     } else {
-        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 0, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        sweep_xy_kernel<XB, LIM, 0, SP><<<grid, threads, smem, st>>>(tm, P);
+        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 0, SP, NV, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        sweep_xy_kernel<XB, LIM, 0, SP, NV, KC><<<grid, threads, smem, st>>>(tm, P);
     }
 }
 
@@ -396,6 +398,12 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     {
         Launch L(c, xfirst ? K_SWEEP_XY : K_SWEEP_YX);
         const bool v32 = s.nv[0] == 32 && s.nv[1] == 32 && s.nv[2] == 32 && xb == 4 && P.PC == C;
+        const int cube = (s.nv[0] == s.nv[1] && s.nv[1] == s.nv[2] && xb == 4 && P.PC == C) ? s.nv[0] : 0;
+        // the other shapes of BASELINE.json's configs 4 and 5
+        if (cube == 24 && G.nx == 64 && C == 8) { if (lim) launch_xy_t<4, 1, 64, 24, 8>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64, 24, 8>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (cube == 48 && G.nx == 64 && C == 16) { if (lim) launch_xy_t<4, 1, 64, 48, 16>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64, 48, 16>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (cube == 40 && G.nx == 256 && C == 8) { if (lim) launch_xy_t<4, 1, 256, 40, 8>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 256, 40, 8>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else
         if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (v32 && G.nx == 64 && C == 32) { if (lim) launch_xy_t<4, 1, 64>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (xb == 8) { if (lim) launch_xy_t<8, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<8, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }

@@ -118,14 +118,17 @@ def test_spatial_half_steps(gpu, orc, bc, stages):
 
 
 @pytest.mark.parametrize("bc,g", [(inputs.BC_PERIODIC, 0), (inputs.BC_REFLECT, 0), (inputs.BC_FLUID, 2), (inputs.BC_FLUID, 3)])
-@pytest.mark.parametrize("nx,nv", [(13, (6, 8, 10)), (12, (4, 4, 8)), (16, (6, 8, 16)), (24, (3, 6, 32))])
+@pytest.mark.parametrize("nx,nv", [(13, (6, 8, 10)), (12, (4, 4, 8)), (16, (6, 8, 16)), (24, (3, 6, 32)),
+                                   (64, (24, 24, 24)), (64, (32, 32, 32)), (128, (32, 32, 32))])
 @pytest.mark.parametrize("stages", [1, 4])
 def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
-    """a1+a2 / a7+a8 as ONE fused pass (all |sigma| < 1): x blocks of 1, 4, 8 cells, chunks of 2..32 velocity cells
+    """a1+a2 / a7+a8 as ONE fused pass (all |sigma| < 1): x blocks of 1 and 4 cells, chunks of 2..32 velocity cells
     made of part of a v_z row / several rows, every y boundary kind; against the oracle and against the general
-    one-direction kernels."""
+    one-direction kernels.  The shapes with nx = 64 / 128 are compile-time-shape kernels of the benchmark configs."""
     rng = np.random.default_rng(5)
-    w = random_workload(rng, nx=nx, ny=7, nv=nv, g=g, bc=bc)
+    w = random_workload(rng, nx=nx, ny=7 if nx < 64 else 3, nv=nv, g=g, bc=bc)
+    if nx >= 64:
+        w.lx = 3.4 * nx / 24      # full velocity grids reach |v_x| = 3.9: keeps |sigma_x| <= 0.7
     f0 = [smooth_random_f(rng, w, 0)]
     Z = np.zeros((3, w.ny_g, w.nx))
     dt = 0.05          # |sigma_x| <= 4 * 0.025 / (1.7/24) = 0.71 ... 0.38; |sigma_y| <= 3 * 0.025 / (0.9/7) = 0.58
