@@ -325,8 +325,11 @@ __global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams
 template <int LIM, int CN>
 __global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
     extern __shared__ __align__(128) double sm[];
-    constexpr int CT = 128, N = CN, plane = CN * CN, ntile = plane / CT, nsegx = CN / 8, seglen = 8;
+    // the last tile of a plane may be ragged (24^2, 40^2: 64 columns; the box is zero-filled past the plane): a
+    // multiple of 32, so warps stay whole
+    constexpr int CT = 128, N = CN, plane = CN * CN, ntile = (plane + CT - 1) / CT, nsegx = CN / 8, seglen = 8;
     constexpr int ROWS = 3 * V_PAD + 2 * CN;
+    static_assert(plane % 32 == 0 && CN % 8 == 0, "whole warps, whole segments");
     // only the three pad strips are ever written by threads (zeros, once); the buffers belong to the TMA unit
     for (int e = threadIdx.x; e < V_PAD * CT; e += V_THREADS) {
         sm[e] = 0.0; sm[(V_PAD + CN) * CT + e] = 0.0; sm[(2 * V_PAD + 2 * CN) * CT + e] = 0.0;
@@ -360,11 +363,12 @@ __global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid
         for (int wi = threadIdx.x; wi < CT * nsegx; wi += V_THREADS) {
             const int seg = wi / CT, c = wi - seg * CT;
             const int col = c0 + c;
+            if (plane % CT != 0 && col >= plane) continue;
             const int k1 = col / CN, k2 = col - k1 * CN;
             const double s0 = t0 + t2 * k1 + t3 * k2;
             const int a = seg * seglen;
             OutGlobal o{fb + c + (long)a * plane, (long)plane};
-            march_cells<LIM, 2>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);     // 512 items, 256 threads: full warps
+            march_cells<LIM, 2>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);     // whole warps take this together
         }
         __syncthreads();                           // everybody is done reading buffer b: refill it
         if (threadIdx.x == 0 && tile + 2 * (int)gridDim.x < P.ntot) issue(tile + 2 * gridDim.x, b);
@@ -620,16 +624,23 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 16) k = lim ? vsweep_x_kernel<1, 16> : vsweep_x_kernel<0, 16>;
         if (spec == 32) k = lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>;
         const int cube32 = spec ? 1 : 0;
-        if (spec && !ghost && (long)c->G.nyg * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
-            // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]
+        const int tspec = (cn == 16 || cn == 24 || cn == 32 || cn == 40 || cn == 48) ? cn : 0;
+        if (tspec && !ghost && (long)c->G.nyg * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
+            // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]; its own tile shape
             CUtensorMap tm;
-            if (!make_tensor_map_2d(&tm, f, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, spec)) return VLASOV_ECUDA;
+            if (!make_tensor_map_2d(&tm, f, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, tspec)) return VLASOV_ECUDA;
+            P.ct = 128; P.nseg = tspec / 8;
+            P.ntile = (plane + 127) / 128;
+            P.ntot = P.ntile * ncell;
             void (*kt)(CUtensorMap, VParams) = lim ? vsweep_x_tma_kernel<1, 32> : vsweep_x_tma_kernel<0, 32>;
-            if (spec == 16) kt = lim ? vsweep_x_tma_kernel<1, 16> : vsweep_x_tma_kernel<0, 16>;
-            const size_t smem_t = (size_t)(3 * V_PAD + 2 * spec) * 128 * 8 + 16;
-            static int occ_t[4] = {0, 0, 0, 0};
-            static size_t occ_t_smem[4] = {0, 0, 0, 0};
-            const int gi = lim + (spec == 16 ? 2 : 0);
+            if (tspec == 16) kt = lim ? vsweep_x_tma_kernel<1, 16> : vsweep_x_tma_kernel<0, 16>;
+            if (tspec == 24) kt = lim ? vsweep_x_tma_kernel<1, 24> : vsweep_x_tma_kernel<0, 24>;
+            if (tspec == 40) kt = lim ? vsweep_x_tma_kernel<1, 40> : vsweep_x_tma_kernel<0, 40>;
+            if (tspec == 48) kt = lim ? vsweep_x_tma_kernel<1, 48> : vsweep_x_tma_kernel<0, 48>;
+            const size_t smem_t = (size_t)(3 * V_PAD + 2 * tspec) * 128 * 8 + 16;
+            static int occ_t[16] = {0};
+            static size_t occ_t_smem[16] = {0};
+            const int gi = lim + 2 * (tspec / 8);
             const int grid = min(P.ntot, resident_ctas(kt, smem_t, occ_t[gi], occ_t_smem[gi]));
             Launch L(c, K_VSWEEP_X);
             kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);

@@ -146,7 +146,8 @@ def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
     assert rel_l2(fg[0], fu[0]) <= TOL1
 
 
-@pytest.mark.parametrize("nv", [(12, 10, 14), (8, 16, 32), (32, 32, 32), (24, 24, 24), (4, 40, 40), (6, 48, 48), (16, 16, 16)])
+@pytest.mark.parametrize("nv", [(12, 10, 14), (8, 16, 32), (32, 32, 32), (24, 24, 24), (4, 40, 40), (6, 48, 48), (16, 16, 16),
+                                (40, 40, 40), (48, 48, 48)])
 @pytest.mark.parametrize("fields_yee", [0, 1])
 def test_velocity_step_multicell_shifts(gpu, orc, fields_yee, nv):
     """a3-a6: strong fields give sign-changing shifts of several cells; Yee gather vs cell-centred.  (12,10,14):
