@@ -506,6 +506,8 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     double* Bf = sm + STG;
     double* A = Bf + BUF;
     const unsigned bar = smem_addr(A + BUF);
+    const double* tab = A + BUF + 2;               // the tile's sweep-table row rides along with the tile (16-byte aligned)
+    static_assert((TAB * 8) % 16 == 0, "bulk copy size");
     // zero: the staging pad rows (never written again), Bf and A entirely (their cells are overwritten per tile)
     for (int e = threadIdx.x; e < SPAD * N2; e += V_THREADS) {
         St[e] = 0.0;
@@ -520,7 +522,8 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     auto issue = [&](int tile) {                   // thread 0 only: ct boxes, one per plane
         const int cell = P.cell0 + tile / P.ntile;
         const int p0 = (tile % P.ntile) * ct;
-        mbar_expect_tx(bar, (unsigned)ct * plane * 8);
+        mbar_expect_tx(bar, (unsigned)ct * plane * 8 + TAB * 8);
+        bulk_g2s(smem_addr(tab), P.table + (long)cell * TAB, TAB * 8, bar);
 #pragma unroll
         for (int p = 0; p < ct; ++p)
             tma_g2s_2d(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2) * 8, &tmap, 0, (cell * P.nv0 + p0 + p) * N1, bar);
@@ -538,10 +541,10 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
         const int cell = P.cell0 + tile / P.ntile;
         const int p0 = (tile % P.ntile) * ct;
         double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
-        const double* T = P.table + (long)cell * TAB;
-        const double ty0 = T[4], ty1 = T[5], ty2 = T[6], ty3 = T[7], finfy = T[13];
-        const double tz0 = T[8], tz1 = T[9], tz2 = T[10], tz3 = T[11], finfz = T[14];
         mbar_wait(bar, it & 1);
+        // the table row arrived with the tile; it is overwritten when the next tile is issued (after the vy sweep)
+        const double ty0 = tab[4], ty1 = tab[5], ty2 = tab[6], ty3 = tab[7], finfy = tab[13];
+        const double tz0 = tab[8], tz1 = tab[9], tz2 = tab[10], tz3 = tab[11], finfz = tab[14];
         {   // vy: line along i_vy (stride N2 in the staging buffer); transverse (plane, i_vz); threads run along z
             constexpr int nl = ct * N2;
             for (int wi = threadIdx.x; wi < nl * nseg; wi += V_THREADS) {
@@ -685,7 +688,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (spec == 40) kt = lim ? vsweep_yz_tma_kernel<1, 40> : vsweep_yz_tma_kernel<0, 40>;
             const size_t srows = 8 + (size_t)pt * (s.nv[1] + 8);
             const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
-            const size_t smem_t = (stg + 2 * buf) * 8 + 16;
+            const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8;
             if (smem_t > V_SMEM_MAX) return VLASOV_EINVAL;
             static int occ_t[16] = {0};
             static size_t occ_t_smem[16] = {0};

@@ -23,6 +23,11 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "DONE:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// 1D bulk copy global -> shared (16-byte aligned, a multiple of 16 bytes), completing on the same kind of barrier
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
 // 2D tiled TMA load: the box at element coordinates (c0 inner, c1 outer) lands dense in shared memory as [outer][inner]
 __device__ __forceinline__ void tma_g2s_2d(unsigned dst, const CUtensorMap* tm, int c0, int c1, unsigned bar) {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
