@@ -219,22 +219,110 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
     }
 }
 
+// Segment of SEG cells with shifts of any size whose lanes keep one flow direction along the segment (CROSS = 0), or
+// change it once where |sigma| < 1 (CROSS = 1).  Walk in the direction of the flow as above, tau = |sigma| along it;
+// nothing is kept in registers, a face reads the three cells around its foot.  Shift identity: with Phi = S + G
+// (S the n whole cells of eqs. 46/47, G the partial cell) and n changing by at most one from face to face,
+//     f_own + S_{m-1} - S_m  =  f0_m            n_m = n_{m-1}
+//                            =  0               n_m = n_{m-1} + 1
+//                            =  f0_m + fm_m     n_m = n_{m-1} - 1
+// (f0_m, fm_m: foot cell of face m and its upstream neighbour, read for G_m anyway), so eq. (38) needs neither the
+// whole-cell sums nor the cell itself.  A face against the flow (CROSS, n = 0 there) reads its foot one cell downstream,
+// mirrored, and its own cell is fp.  The last face of the box carries no flux (R7): its S is added back, cell by cell.
+//   flow cell c <-> cell a+c (sigma >= 0) | a+SEG-1-c (sigma < 0);  walk face m lies between flow cells m-1 and m.
+template <int SEG, int LIM, int FULL, int CROSS, class Out>
+__device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
+                                               double s1, double finf, Out out) {
+    const double M = 6755399441055744.0;
+    const bool pos = !(sig_a < 0.0 || sig_b < 0.0);
+    const int u = pos ? st8 : -st8;
+    unsigned fb = L + (pos ? a - 1 : a + SEG) * st8;     // flow cell m-1
+    double tau = pos ? sig_a : -sig_b;                   // tau_m = tau_0 + m s1 in either direction
+    const bool zero_first = pos ? a == 0 : a + SEG == N;
+    const bool zero_last = pos ? a + SEG == N : a == 0;
+    if (!pos) { out.skip(SEG - 1); }
+    out.step(pos ? 1 : -1);
+    double Gp = 0.0;
+    int np = 0;
+    // three faces per trip of a rolled loop: the walks of a sweep must share the 32 KB instruction cache
+#pragma unroll 3
+    for (int m = 0; m <= SEG; ++m) {
+        const double at = fabs(tau);
+        const double r = __dadd_rd(at, M);
+        const int n = __double2loint(r);
+        const double bq = at - (r - M);
+        unsigned F = fb - n * u;                         // foot: flow cell m-1-n
+        int uu = u;
+        bool against = false;
+        double bs = bq;                                  // bq with the sign of tau
+        if (CROSS) {
+            const int th = __double2hiint(tau);
+            against = th < 0;
+            F = against ? fb + u : F;                    // n = 0 there: foot = flow cell m, mirrored
+            uu = against ? -u : u;
+            bs = __hiloint2double(__double2hiint(bq) | (th & 0x80000000), __double2loint(bq));
+        }
+        const double f0 = lds(F), fm = lds(F - uu), fp = lds(F + uu);
+        double sp, sm;
+        slopes_fast<LIM, FULL>(fm, f0, fp, finf, sp, sm);
+        const double b2 = bq * bq;
+        const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
+        const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+        double G = bs * fma(c1, sp, fma(c2, sm, f0));
+        if (m == 0) {
+            if (zero_first) G = 0.0;
+        } else {
+            double T = f0;
+            if (__any_sync(FULL ? 0xffffffffu : __activemask(), n != np)) {      // a quarter of the faces of a warp
+                if (n > np) T = 0.0;
+                if (n < np) T = f0 + fm;
+            }
+            if (CROSS && against) T = fp;
+            if (m == SEG && zero_last) {
+                G = 0.0;
+                unsigned w = fb;
+#pragma unroll 1
+                for (int l = 0; l < n; ++l) { T += lds(w); w -= u; }
+            }
+            out.put(T + (Gp - G));
+        }
+        Gp = G;
+        np = n;
+        tau += s1;
+        fb += u;
+    }
+}
+
 // One thread remaps cells [a, b) of one line: flux per face, eq. (38) per cell.  sigma of face k is
 // s0 + s1 k (accumulated).  out.put(value) stores the new average of the next cell (a, a+1, ...).
-template <int LIM, int FAST, class Out>
+// FAST: 8-cell segments may take the flow-ordered walks (2: every lane of the warp is here).  LOOSE: the 4th cell
+// before a line is readable memory (any value), which admits floor|sigma| = 2 at a box face.
+template <int LIM, int FAST, int LOOSE = 0, class Out>
 __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
                                             double finf, Out& out) {
     double sig = fma(s1, (double)a, s0);
     constexpr int SEG = 8;
     if (FAST && b - a == SEG) {
         // sigma is affine along the line: |sigma| < 1 and one sign at both end faces hold on every face between.
-        // (A register-window walk for multi-cell shifts was built and measured: its whole-cell sum loops cost what
-        // the general walk's addressing costs -- DESIGN.md section 11.)
         const double sig_b = fma(s1, (double)b, s0);
-        const bool small = fabs(sig) < 1.0 && fabs(sig_b) < 1.0 && !(sig * sig_b < 0.0);
+        const bool cross = sig * sig_b < 0.0;
+        const bool sub = fabs(sig) < 1.0 && fabs(sig_b) < 1.0;
         constexpr int FULL = FAST == 2 ? 1 : 0;        // FAST == 2: every lane of the warp is here
-        if (__all_sync(FULL ? 0xffffffffu : __activemask(), small)) {
+        const unsigned mask = FULL ? 0xffffffffu : __activemask();
+        if (__all_sync(mask, sub && !cross)) {
             march_seg_small<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            return;
+        }
+        // march_seg_lite: its first face reads flow cells -3-n .. -1-n, with V_PAD zero cells before the line; the
+        // reads of a box face are discarded (zero flux), and n grows by less than 1/2 per face
+        const bool pos = !(sig < 0.0 || sig_b < 0.0);
+        const double t0 = pos ? sig : sig_b;
+        const int dist = pos ? a : N - b;              // cells between the box face and the first face of the walk
+        const double bound = (LOOSE && dist == 0) ? (double)V_PAD - 0.5 : (double)(min(dist, 32) + V_PAD - 1);
+        const bool lite = fabs(t0) < bound && fabs(s1) <= 0.5 && (!cross || sub);
+        if (__all_sync(mask, lite)) {
+            if (__any_sync(mask, cross)) march_seg_lite<SEG, LIM, FULL, 1>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            else march_seg_lite<SEG, LIM, FULL, 0>(L, st8, N, a, sig, sig_b, s1, finf, out);
             return;
         }
     }
@@ -553,7 +641,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
                 const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
                 const int a = seg * seglen, b = min(a + seglen, N1);
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM, FW>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+                march_cells<LIM, FW, 1>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
@@ -566,7 +654,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
                 const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
                 const int a = seg * seglen, b = min(a + seglen, N2);
                 OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
-                march_cells<LIM, FW>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
+                march_cells<LIM, FW, 1>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
             }
         }
         __syncthreads();                           // vz done: A complete
