@@ -607,16 +607,17 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
     const unsigned sSt = smem_addr(St), sA = smem_addr(A);
-    auto issue = [&](int tile) {                   // thread 0 only: ct boxes, one per plane
-        const int cell = P.cell0 + tile / P.ntile;
-        const int p0 = (tile % P.ntile) * ct;
+    auto issue = [&](int cell, int p0) {           // thread 0 only: ct boxes, one per plane
         mbar_expect_tx(bar, (unsigned)ct * plane * 8 + TAB * 8);
         bulk_g2s(smem_addr(tab), P.table + (long)cell * TAB, TAB * 8, bar);
 #pragma unroll
         for (int p = 0; p < ct; ++p)
             tma_g2s_2d(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2) * 8, &tmap, 0, (cell * P.nv0 + p0 + p) * N1, bar);
     };
-    if (threadIdx.x == 0 && (int)blockIdx.x < P.ntot) issue(blockIdx.x);
+    // (spatial cell, tile within the cell) of this CTA's tiles, advanced without a division per tile
+    const int step_c = gridDim.x / P.ntile, step_t = gridDim.x % P.ntile;
+    int tcell = blockIdx.x / P.ntile, ttile = blockIdx.x % P.ntile;
+    if (threadIdx.x == 0 && (int)blockIdx.x < P.ntot) issue(P.cell0 + tcell, ttile * ct);
     // staging map of the store loop (as in the plain kernel)
     const int z_init = threadIdx.x % N2, row_init = threadIdx.x / N2;
     const int y_init = row_init % N1;
@@ -626,9 +627,11 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     constexpr int ncellt = ct * plane;
     int it = 0;
     for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x, ++it) {
-        const int cell = P.cell0 + tile / P.ntile;
-        const int p0 = (tile % P.ntile) * ct;
+        const int cell = P.cell0 + tcell;
+        const int p0 = ttile * ct;
         double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
+        tcell += step_c; ttile += step_t;
+        if (ttile >= P.ntile) { ttile -= P.ntile; ++tcell; }
         mbar_wait(bar, it & 1);
         // the table row arrived with the tile; it is overwritten when the next tile is issued (after the vy sweep)
         const double ty0 = tab[4], ty1 = tab[5], ty2 = tab[6], ty3 = tab[7], finfy = tab[13];
@@ -645,7 +648,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
-        if (threadIdx.x == 0 && tile + (int)gridDim.x < P.ntot) issue(tile + gridDim.x);
+        if (threadIdx.x == 0 && tile + (int)gridDim.x < P.ntot) issue(P.cell0 + tcell, ttile * ct);
         {   // vz: contiguous lines of Bf; transverse (plane, i_vy); threads run along y (pitch RS, odd)
             constexpr int nl = ct * N1;
             for (int wi = threadIdx.x; wi < nl * nseg; wi += V_THREADS) {
