@@ -171,6 +171,32 @@ def test_velocity_step_multicell_shifts(gpu, orc, fields_yee, nv):
     assert np.abs(fg[0] - f0[0]).max() > 0.1
 
 
+@pytest.mark.parametrize("nv", [(32, 32, 32), (24, 24, 24), (16, 16, 16), (48, 48, 48), (8, 16, 32)])
+@pytest.mark.parametrize("limiter", [1, 0])
+def test_velocity_step_moderate_rotation(gpu, orc, limiter, nv):
+    """a3-a6 in the regime of the GEM electrons: rotation angles of 0.03 .. 0.25 per step, so sigma is nearly constant
+    along a line (slope of a few hundredths per face) but reaches 0.5 .. 4 cells at the edge of the box, changes sign
+    inside segments, and floor|sigma| steps by one inside segments.  This is what the flow-ordered walk for
+    multi-cell shifts (shift identity) takes: box faces with floor|sigma| = 1, 2 (the whole
+    cells added back at the outflow face), crossing lanes, both limiter settings (without the limiter the flux of
+    the inflow box face is zeroed explicitly); 32 / 16: TMA kernels with whole warps, 24: partial warps, 48 and
+    (8,16,32): the plain kernels, which admit one cell less before a line."""
+    rng = np.random.default_rng(11)
+    w = random_workload(rng, nx=4, ny=2, nv=nv, bc=inputs.BC_REFLECT, fields_yee=1)
+    f0 = [smooth_random_f(rng, w, 0)]
+    E = 2.0 * rng.standard_normal((3, w.ny_g, w.nx))
+    B = rng.standard_normal((3, w.ny_g, w.nx))
+    B *= rng.uniform(0.3, 2.5, size=(1, w.ny_g, w.nx)) / np.sqrt((B ** 2).sum(0, keepdims=True))
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, 0.1, 2, limiter=limiter)
+    assert code == 0
+    assert rel_l2(fg[0], fo[0]) <= TOL1
+    assert np.abs(fg[0] - fo[0]).max() <= 1e-13
+    assert rel_l2(mg[0], mo[0]) <= TOL1
+    m0 = f0[0].sum()
+    assert abs(fg[0].sum() - m0) / m0 <= 1e-13      # zero flux through the box faces (R7)
+    assert np.abs(fg[0] - f0[0]).max() > 0.1
+
+
 @pytest.mark.parametrize("order", [0, 1])
 @pytest.mark.parametrize("limiter", [1, 0])
 def test_full_step_two_species(gpu, orc, order, limiter):
