@@ -183,7 +183,7 @@ __device__ __forceinline__ int need_bits(double f0, double dp, double dm, double
 // Segment of SEG cells [a, a+SEG) whose SEG+1 faces all have |sigma| < 1 (no whole cells in eqs. 46/47) and one
 // flow direction: the SEG+3 cells the fluxes touch are read ONCE into registers, in the direction of the flow
 // (eq. 47 = eq. 46 on the mirrored line), and face m of the walk takes (q[m], q[m+1], q[m+2]).  About a
-// quarter of the instructions of the general walk below (DESIGN.md "Velocity sweeps: segment fast path").
+// quarter of the instructions of the general walk below (DESIGN.md "Flow-ordered walks").
 //   walk position i <-> cell a-2+i (sigma >= 0) | a+SEG+1-i (sigma < 0);  face m <-> face a+m | a+SEG-m.
 template <int SEG, int LIM, int FULL, class Out>
 __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
