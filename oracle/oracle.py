@@ -160,6 +160,18 @@ def moments(f, sp, nx, ny, g):
     return mom
 
 
+def fluid_boundary(f_t, f_t1, sp, nx, ny, g, side, theta):
+    """Section 4.1: boundary data for the two-fluid code.  The raw moments, eqs. (2)-(4), of the g
+    kinetic rows next to the border `side` (0: rows 0..g-1 of the interior, 1: rows ny-g..ny-1; reading R22: the fluid
+    block's ghost cells are as deep as the kinetic block's), at time t + theta dt "by linear interpolation in time"
+    between the Vlasov data at t (f_t) and at t + dt (f_t1).  Returns [10][g][nx]."""
+    assert g >= 1 and ny >= g and side in (0, 1)
+    j0 = g if side == 0 else ny            # ghost-inclusive index of the first of those rows
+    m_t = moments(f_t, sp, nx, ny, g)[:, j0:j0 + g, :]
+    m_t1 = moments(f_t1, sp, nx, ny, g)[:, j0:j0 + g, :]
+    return (1.0 - theta) * m_t + theta * m_t1
+
+
 def ghost_fill(f, sp, nx, ny, g, side, fluid5, limiter=1):
     assert f.flags.c_contiguous and f.dtype == np.float64
     fluid5 = _f64(fluid5)

@@ -233,3 +233,45 @@ def test_eq11_current_from_moments(orc):
     Jy = orc.current([m1], [1.0], fields_yee=1, wall=1)
     assert np.allclose(Jy[0, 1:], yc[1:] - 0.5) and np.allclose(Jy[1], 2 * yc) and np.allclose(Jy[2, 1:], 3 * (yc[1:] - 0.5))
     assert not Jy[0, 0].any() and not Jy[2, 0].any()
+
+
+@pytest.mark.parametrize("side", [0, 1])
+def test_T17_fluid_boundary_rows_moments_and_time_interpolation(orc, side):
+    """Section 4.1: the fluid code's boundary data are the moments (eqs. 2-4) of the kinetic rows next
+    to the border, linearly interpolated in time.  Pinned against brute-force sums written here (not the oracle's
+    moment routine) on data where every row, column and time level is different, so a wrong row, side, moment index
+    or weight fails; and against the closed form for drifting Maxwellians whose density changes in time."""
+    nv, g, nx, ny = (8, 6, 10), 2, 3, 5
+    vmin, vmax = (-5.0, -4.0, -6.0), (5.0, 4.0, 6.0)
+    sp = orc.Species(-1.0, 1.0, nv, vmin, vmax, 1.0)
+    rng = np.random.default_rng(5)
+    f_t = rng.random((ny + 2 * g, nx) + nv)
+    f_t1 = rng.random((ny + 2 * g, nx) + nv)
+    dv = [(vmax[d] - vmin[d]) / nv[d] for d in range(3)]
+    c = [vmin[d] + (np.arange(nv[d]) + 0.5) * dv[d] for d in range(3)]
+    V = np.meshgrid(*c, indexing="ij")
+    w = dv[0] * dv[1] * dv[2]
+    rows = range(g, 2 * g) if side == 0 else range(ny, ny + g)       # ghost-inclusive indices of the g interior rows
+    pairs = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]         # M2 order xx yy zz xy xz yz (vlasov.h)
+    for theta in (0.0, 0.5, 0.3, 1.0):
+        got = orc.fluid_boundary(f_t, f_t1, sp, nx, ny, g, side, theta)
+        assert got.shape == (10, g, nx)
+        for l, j in enumerate(rows):
+            for i in range(nx):
+                fb = (1.0 - theta) * f_t[j, i] + theta * f_t1[j, i]      # moments are linear in f
+                want = [fb.sum() * w] + [(fb * V[d]).sum() * w for d in range(3)] + \
+                       [(fb * V[a] * V[b]).sum() * w for a, b in pairs]
+                np.testing.assert_allclose(got[:, l, i], want, rtol=1e-12, atol=1e-10)   # odd moments cancel: sums of terms of size 1e3
+    # closed form: Maxwellians, density 1 at t and 3 at t + dt, drift (0.3, -0.2, 0.1), T = 0.5: M0 = 1 + 2 theta,
+    # M1 = M0 V, trace M2 = M0 (3 T + V^2) up to the midpoint-rule error (spectrally small for a resolved Gaussian)
+    nv2 = (24, 24, 24)
+    sp2 = orc.Species(1.0, 1.0, nv2, (-6.0,) * 3, (6.0,) * 3, 1.0)
+    Vd, T = (0.3, -0.2, 0.1), (0.5, 0.5, 0.5)
+    blk = _maxw_block(24, (-6.0,) * 3, (6.0,) * 3, 1.0, Vd, T)
+    a = np.zeros((ny + 2 * g, nx) + nv2); b = np.zeros_like(a)
+    a[g:g + ny] = blk; b[g:g + ny] = 3.0 * blk
+    got = orc.fluid_boundary(a, b, sp2, nx, ny, g, side, 0.25)
+    np.testing.assert_allclose(got[0], 1.5, rtol=1e-9)
+    for d in range(3):
+        np.testing.assert_allclose(got[1 + d], 1.5 * Vd[d], rtol=1e-8)
+    np.testing.assert_allclose(got[4] + got[5] + got[6], 1.5 * (1.5 + sum(v * v for v in Vd)), rtol=1e-8)
