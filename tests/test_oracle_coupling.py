@@ -267,7 +267,7 @@ def test_T17_fluid_boundary_rows_moments_and_time_interpolation(orc, side):
     nv2 = (24, 24, 24)
     sp2 = orc.Species(1.0, 1.0, nv2, (-6.0,) * 3, (6.0,) * 3, 1.0)
     Vd, T = (0.3, -0.2, 0.1), (0.5, 0.5, 0.5)
-    blk = _maxw_block(24, (-6.0,) * 3, (6.0,) * 3, 1.0, Vd, T)
+    blk = _maxw_block(nv2, (-6.0,) * 3, (6.0,) * 3, 1.0, Vd, T)
     a = np.zeros((ny + 2 * g, nx) + nv2); b = np.zeros_like(a)
     a[g:g + ny] = blk; b[g:g + ny] = 3.0 * blk
     got = orc.fluid_boundary(a, b, sp2, nx, ny, g, side, 0.25)
