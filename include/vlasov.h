@@ -117,6 +117,21 @@ int vlasov_step_host(vlasov_ctx* ctx, double dt, const double* E_host, const dou
  * (vlasov_touch), the kept result is copied; otherwise f is reduced again. */
 int vlasov_moments(vlasov_ctx* ctx, int species, double* mom_dev /*[10][ny_g][nx]*/);
 
+/* Boundary data for the two-fluid code, section 4.1: "the boundary data needed by the two-fluid code
+ * can be calculated by means of the moment equations (2)-(4) ... needs boundary conditions at times t, t + dt/2 and
+ * t + dt.  Thus the Vlasov data has to be advanced before the fluid data.  Then, by linear interpolation in time, the
+ * intermediate boundary conditions can be calculated".
+ * vlasov_fluid_boundary_mark: call at time t, before the step: keeps the raw moments (layout and order of
+ *   vlasov_moments) of the nghost_y interior rows next to both y borders, for every species (reading R22: the fluid
+ *   block's ghost cells are as deep as the kinetic block's).
+ * vlasov_fluid_boundary: call after the step: reduces the same rows of the current f and writes
+ *   (1 - theta) * marked + theta * current to out_dev [10][nghost_y][nx] (row l = l-th of those rows in ascending y;
+ *   side 0 = y_lo: interior rows 0..g-1, side 1 = y_hi: interior rows ny-g..ny-1).  theta in [0,1] is not enforced
+ *   (extrapolation is the caller's business).
+ * Errors: EINVAL (nghost_y == 0, ny < nghost_y, bad species/side, no mark yet, NULL), EALIGN. */
+int vlasov_fluid_boundary_mark(vlasov_ctx* ctx);
+int vlasov_fluid_boundary(vlasov_ctx* ctx, int species, int side, double theta, double* out_dev /*[10][g][nx]*/);
+
 /* Current density j = sum_s q_s M1^(s), eq. (11), at cell centres or (fields_yee)
  * linearly interpolated to the E positions of R17. */
 int vlasov_current(vlasov_ctx* ctx, double* J_dev /*[3][ny_g][nx]*/);

@@ -18,7 +18,7 @@ STAGE_X1, STAGE_V, STAGE_X2, STAGE_GHOST, STAGE_MOMENTS, STAGE_ALL = 1, 2, 4, 8,
 EXPORTS = ["vlasov_scratch_bytes", "vlasov_init", "vlasov_set_boundary", "vlasov_step", "vlasov_step_host",
            "vlasov_moments", "vlasov_current", "vlasov_maxwell", "vlasov_touch", "vlasov_set_option", "vlasov_check",
            "vlasov_launch_count", "vlasov_free", "vlasov_strerror", "vlasov_cycle", "vlasov_cycle_host",
-           "vlasov_timing_enable", "vlasov_timing_read"]
+           "vlasov_timing_enable", "vlasov_timing_read", "vlasov_fluid_boundary_mark", "vlasov_fluid_boundary"]
 OPT_FUSE_XY = 1
 KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy", "sweep_yx"]
 
@@ -66,6 +66,10 @@ def lib():
         L.vlasov_step_host.argtypes = [vp, C.c_double, dp, dp, C.c_uint32, dp]
         L.vlasov_moments.restype = C.c_int
         L.vlasov_moments.argtypes = [vp, C.c_int, dp]
+        L.vlasov_fluid_boundary_mark.restype = C.c_int
+        L.vlasov_fluid_boundary_mark.argtypes = [vp]
+        L.vlasov_fluid_boundary.restype = C.c_int
+        L.vlasov_fluid_boundary.argtypes = [vp, C.c_int, C.c_int, C.c_double, dp]
         L.vlasov_current.restype = C.c_int
         L.vlasov_current.argtypes = [vp, dp]
         L.vlasov_maxwell.restype = C.c_int
@@ -179,6 +183,12 @@ class Context:
 
     def vlasov_moments(self, species, mom):
         _chk(lib().vlasov_moments(self.h, species, _ptr(mom)), "vlasov_moments")
+
+    def vlasov_fluid_boundary_mark(self):
+        _chk(lib().vlasov_fluid_boundary_mark(self.h), "vlasov_fluid_boundary_mark")
+
+    def vlasov_fluid_boundary(self, species, side, theta, out):
+        _chk(lib().vlasov_fluid_boundary(self.h, int(species), int(side), float(theta), _ptr(out)), "vlasov_fluid_boundary")
 
     def vlasov_current(self, J):
         _chk(lib().vlasov_current(self.h, _ptr(J)), "vlasov_current")

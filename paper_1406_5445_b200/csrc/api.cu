@@ -11,7 +11,7 @@ namespace {
 inline size_t align_up(size_t x) { return (x + 127) & ~(size_t)127; }
 
 struct Carve {
-    size_t pong, table, mom, gmom, fields, jbuf, bavg, err, total;
+    size_t pong, table, mom, gmom, bmark, bcur, fields, jbuf, bavg, err, total;
 };
 
 bool carve(const vlasov_config* cfg, const vlasov_species* sp, Carve& C) {
@@ -30,6 +30,8 @@ bool carve(const vlasov_config* cfg, const vlasov_species* sp, Carve& C) {
     C.table = off;  off += align_up(ncell * TAB * 8);
     C.mom = off;    off += align_up((size_t)cfg->nspecies * 11 * ncell * 8);
     C.gmom = off;   off += align_up((size_t)11 * cfg->nx * 8);
+    C.bmark = off;  off += align_up((size_t)cfg->nspecies * 2 * 11 * cfg->nghost_y * cfg->nx * 8);
+    C.bcur = off;   off += align_up((size_t)11 * cfg->nghost_y * cfg->nx * 8);
     C.fields = off; off += align_up(6 * ncell * 8);
     C.jbuf = off;   off += align_up(3 * ncell * 8);
     C.bavg = off;   off += align_up(3 * ncell * 8);
@@ -161,6 +163,9 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     c->table = (double*)(base + C.table);
     c->mom = (double*)(base + C.mom);
     c->gmom = (double*)(base + C.gmom);
+    c->bmark = (double*)(base + C.bmark);
+    c->bcur = (double*)(base + C.bcur);
+    c->bmark_valid = 0;
     c->fields_stage = (double*)(base + C.fields);
     c->Jbuf = (double*)(base + C.jbuf);
     c->Bavg = (double*)(base + C.bavg);
@@ -290,6 +295,32 @@ int vlasov_moments(vlasov_ctx* c, int species, double* mom_dev) {
     VL_CUDA_OK(cudaMemcpyAsync(mom_dev, c->mom + (size_t)species * 11 * ncell, 10 * ncell * 8,
                                cudaMemcpyDeviceToDevice, c->stream));
     return VLASOV_OK;
+}
+
+// Section 4.1: the g interior rows next to border `side`, ghost-inclusive index of the first one
+static inline int border_row0(const Geom& G, int side) { return side == 0 ? G.g : G.ny; }
+
+int vlasov_fluid_boundary_mark(vlasov_ctx* c) {
+    if (!c || c->G.g < 1 || c->G.ny < c->G.g) return VLASOV_EINVAL;
+    const size_t n = (size_t)c->G.g * c->G.nx;
+    for (int s = 0; s < c->ns; ++s)
+        for (int side = 0; side < 2; ++side) {
+            int e = launch_moments(c, c->sp[s], c->sp[s].f, c->bmark + ((size_t)(s * 2 + side) * 11) * n,
+                                   border_row0(c->G, side), c->G.g);
+            if (e) return e;
+        }
+    c->bmark_valid = 1;
+    return VLASOV_OK;
+}
+
+int vlasov_fluid_boundary(vlasov_ctx* c, int species, int side, double theta, double* out_dev) {
+    if (!c || species < 0 || species >= c->ns || side < 0 || side > 1 || !out_dev) return VLASOV_EINVAL;
+    if (c->G.g < 1 || c->G.ny < c->G.g || !c->bmark_valid) return VLASOV_EINVAL;
+    if (((uintptr_t)out_dev) & 7) return VLASOV_EALIGN;
+    const size_t n = (size_t)c->G.g * c->G.nx;
+    int e = launch_moments(c, c->sp[species], c->sp[species].f, c->bcur, border_row0(c->G, side), c->G.g);
+    if (e) return e;
+    return launch_lerp(c, c->bmark + ((size_t)(species * 2 + side) * 11) * n, c->bcur, theta, out_dev, (long)(10 * n));
 }
 
 int vlasov_current(vlasov_ctx* c, double* J_dev) {

@@ -102,6 +102,24 @@ int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out
 }
 
 // ------------------------------------------------------------------------------------------------
+// Section 4.1: "by linear interpolation in time": out = (1 - theta) a + theta b, two products and a
+// sum, each rounded (no contraction), as the oracle writes it.
+// ------------------------------------------------------------------------------------------------
+__global__ void lerp_kernel(const double* __restrict__ a, const double* __restrict__ b, double theta, double* __restrict__ out, long n) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = __dadd_rn(__dmul_rn(1.0 - theta, a[i]), __dmul_rn(theta, b[i]));
+}
+
+int launch_lerp(vlasov_ctx* c, const double* a, const double* b, double theta, double* out, long n) {
+    if (n <= 0) return VLASOV_OK;
+    {
+        Launch L(c, K_MOMENTS);
+        lerp_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(a, b, theta, out, n);
+    }
+    return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
+}
+
+// ------------------------------------------------------------------------------------------------
 // eq. (11): j = sum_s q_s M1^(s); Yee: interpolated to the E positions of R17
 // ------------------------------------------------------------------------------------------------
 struct CurParams {

@@ -47,6 +47,9 @@ struct vlasov_ctx {
     double* table;       // [nyg*nx][TAB] sweep table (rebuilt per species and stage)
     double* mom;         // [ns][11][nyg*nx] kept moments (+ max f as the 11th)
     double* gmom;        // [11][nx] moments of one edge row (ghost fill)
+    double* bmark;       // [ns][2][11][g*nx] moments of the border rows at the marked time (section 4.1)
+    double* bcur;        // [11][g*nx] the same rows now
+    int bmark_valid;
     double* fields_stage;// [6][nyg*nx] device staging of E,B for vlasov_step_host
     int* errflag;        // device int: first asynchronous error
     int mom_valid;
@@ -102,6 +105,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
 int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out, int row0, int nrows);
 // ghost fill (a0) of one side
 int launch_ghost_fill(vlasov_ctx* c, const Species& s, double* f, int side);
+int launch_lerp(vlasov_ctx* c, const double* a, const double* b, double theta, double* out, long n);
 int launch_current(vlasov_ctx* c, double* J);
 int launch_maxwell(vlasov_ctx* c, double dt, int nsub, double* E, double* B, const double* J, double* Bavg);
 

@@ -62,8 +62,9 @@ def smooth_random_f(rng, w, s):
     return np.ascontiguousarray(f)
 
 
-def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None, fuse=None):
-    """One vlasov_step on both sides.  Returns (f_gpu list, f_orc list, mom_gpu list, mom_orc list, code)."""
+def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None, fuse=None, mark_theta=None):
+    """One vlasov_step on both sides.  Returns (f_gpu list, f_orc list, mom_gpu list, mom_orc list, code).
+    mark_theta: also take the fluid boundary data of section 4.1 around the step (run_both.boundary[s][side] = (gpu, oracle))."""
     import torch
     fg = [dev(f) for f in f0]
     ctx = gpu.context_for(w, fg, order=order, limiter=limiter)
@@ -78,6 +79,8 @@ def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None, 
                 keep.append(t)
                 ctx.vlasov_set_boundary(s, side, inputs.BC_FLUID, t)
     Ed, Bd = dev(E), dev(B)
+    if mark_theta is not None:
+        ctx.vlasov_fluid_boundary_mark()
     ctx.vlasov_step(dt, Ed, Bd, stages)
     code = ctx.check_code()
     run_both.kinds = ctx.vlasov_timing_read()
@@ -96,6 +99,16 @@ def run_both(gpu, orc, w, f0, E, B, dt, stages, order=0, limiter=1, fluid=None, 
                           stages=stages, want_moments=False)
         fo.append(f)
         momo.append(orc.moments(f, osp(orc, spec), w.nx, w.ny, w.nghost_y))
+    if mark_theta is not None:
+        run_both.boundary = []
+        for s, spec in enumerate(w.species):
+            per_side = []
+            for side in (0, 1):
+                b = torch.empty((10, w.nghost_y, w.nx), dtype=torch.float64, device="cuda")
+                ctx.vlasov_fluid_boundary(s, side, mark_theta, b)
+                per_side.append((b.cpu().numpy(), orc.fluid_boundary(f0[s], fo[s], osp(orc, spec), w.nx, w.ny, w.nghost_y,
+                                                                     side, mark_theta)))
+            run_both.boundary.append(per_side)
     out = [t.cpu().numpy() for t in fg]
     ctx.close()
     return out, fo, momg, momo, code
@@ -250,11 +263,16 @@ def test_ghost_fill_band(gpu, orc):
             assert np.abs(fg[s][rows] - f0[s][rows]).max() > 0          # it did something
         assert np.array_equal(fg[s][g:g + w.ny], f0[s][g:g + w.ny])     # interior untouched
     # whole step with ghost rows as Dirichlet data
-    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, w.dt, 31, fluid=fluid)
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, w.dt, 31, fluid=fluid, mark_theta=0.5)
     assert code == 0
     for s in range(2):
         assert rel_l2(fg[s], fo[s]) <= TOL1
         assert rel_l2(mg[s], mo[s]) <= TOL1
+        # the other direction of the coupling (section 4.1): boundary data for the fluid code at t + dt/2
+        for side in (0, 1):
+            got, want = run_both.boundary[s][side]
+            assert rel_l2(got, want) <= TOL1
+            assert np.abs(want[0]).min() > 0
 
 
 def test_free_streaming_integer_shifts_exact_on_gpu(gpu):
@@ -376,6 +394,46 @@ def test_maxwell_and_current(gpu, orc):
         assert rel_l2(Bd.cpu().numpy(), Bo) <= 1e-14
         assert rel_l2(Bavg.cpu().numpy(), Bavg_o) <= 1e-14
         ctx.close()
+
+
+@pytest.mark.parametrize("g", [1, 3])
+def test_fluid_boundary_data(gpu, orc, g):
+    """Section 4.1 (NEXT-2's Vlasov -> fluid half): moments of the g kinetic rows next to either border,
+    marked at t, reduced again at t + dt, interpolated linearly in time; two species, both sides, theta inside and at
+    the ends of [0, 1]; the call before any mark and on a context without ghost rows is refused."""
+    import torch
+    rng = np.random.default_rng(12)
+    w = random_workload(rng, nx=5, ny=7, nv=(8, 6, 10), g=g, bc=inputs.BC_FLUID, nspecies=2)
+    f_t = [smooth_random_f(rng, w, s) for s in range(2)]
+    f_t1 = [smooth_random_f(rng, w, s) * rng.uniform(0.5, 1.0) for s in range(2)]
+    fg = [dev(f) for f in f_t]
+    ctx = gpu.context_for(w, fg)
+    out = torch.zeros((10, g, w.nx), dtype=torch.float64, device="cuda")
+    with pytest.raises(gpu.VlasovError) as e:
+        ctx.vlasov_fluid_boundary(0, 0, 0.5, out)
+    assert e.value.code == gpu.EINVAL
+    ctx.vlasov_fluid_boundary_mark()
+    for s in range(2):
+        fg[s].copy_(dev(f_t1[s]))                  # "the Vlasov data has to be advanced before the fluid data"
+    ctx.vlasov_touch()
+    for s in range(2):
+        sp = osp(orc, w.species[s])
+        for side in (0, 1):
+            for theta in (0.0, 0.3, 0.5, 1.0):
+                ctx.vlasov_fluid_boundary(s, side, theta, out)
+                assert ctx.check_code() == 0
+                want = orc.fluid_boundary(f_t[s], f_t1[s], sp, w.nx, w.ny, g, side, theta)
+                assert rel_l2(out.cpu().numpy(), want) <= TOL1, (s, side, theta)
+    with pytest.raises(gpu.VlasovError):
+        ctx.vlasov_fluid_boundary(2, 0, 0.5, out)
+    ctx.close()
+    w0 = random_workload(rng, nx=4, ny=4, nv=(4, 4, 4), g=0, bc=inputs.BC_PERIODIC)
+    f0 = [dev(smooth_random_f(rng, w0, 0))]
+    ctx = gpu.context_for(w0, f0)
+    with pytest.raises(gpu.VlasovError) as e:
+        ctx.vlasov_fluid_boundary_mark()
+    assert e.value.code == gpu.EINVAL
+    ctx.close()
 
 
 def test_error_paths(gpu, orc):
