@@ -7,10 +7,14 @@
 // A tiny kernel fills that table from E, B (a3); the ghost fill (section 4.2, eq. 63) writes the same
 // table with its own affine map, so one set of sweep kernels serves both.
 //
-// Sweep kernels: the tile of lines is staged in shared memory, ONE THREAD PER FACE computes the flux
-// of eqs. (46)/(47) (multi-cell, sign-changing shifts; zero flux through the two box faces, R7) into a
-// second shared array, then every cell is updated by eq. (38).  vx: tile = all i_vx x 128 contiguous
-// (i_vy,i_vz) cells.  vy+vz fused: tile = a few contiguous i_vx planes.  In place on f.
+// Sweep kernels: the tile of lines is staged in shared memory (tiled TMA for the compile-time shapes, cp.async
+// otherwise) between zero pad cells (f = 0 outside the box, R7), and ONE THREAD WALKS A SEGMENT of about 8 cells of
+// one line: flux of eqs. (46)/(47) per face, eq. (38) per cell, zero flux through the two box faces.  Three walks,
+// picked per warp by vote: march_seg_small (|sigma| < 1: the cells of the segment
+// live in registers), march_seg_lite (shifts of several cells, sign changes: shift identity, no whole-cell sums),
+// and the general per-face walk of march_cells.  vx: tile = all i_vx x 128 contiguous (i_vy,i_vz) cells, results
+// straight to global memory.  vy+vz fused: tile = a few contiguous i_vx planes, vy: staging -> Bf, vz: Bf -> A,
+// A -> global.  In place on f.
 #include "vlasov_internal.cuh"
 #include "tma.cuh"
 
