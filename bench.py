@@ -394,6 +394,10 @@ def gpu_arm(args):
         "cpu_baseline": cpu,
     }
     out["step_hbm"]["frac_of_peak"] = out["step_hbm"]["achieved_gbs"] / peak
+    # SURVEY.md 8(d) reporting rule: the same figure against the nominal 8 TB/s, and the "useful" fraction that
+    # credits only the 48 B per cell-update of the 3-pass Strang floor (x/2 y/2, V, y/2 x/2 each once through HBM)
+    out["step_hbm"]["frac_of_nominal_8tbs"] = out["step_hbm"]["achieved_gbs"] / 8000.0
+    out["step_hbm"]["useful_frac_48B"] = 48.0 * value / max(world, 1) / 1e9 / peak
     print(json.dumps(out))
     ctx.close()
     if dist is not None:
