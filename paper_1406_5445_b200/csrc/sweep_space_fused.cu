@@ -15,7 +15,6 @@
 //     previous flux per owned cell.
 // Rows -2, -1 and ny, ny+1 are the boundary rows of the y sweep (R16, R19): periodic wrap, the wall
 // image f(y_w + eta, vy) = f(y_w - eta, -vy), or FLUID ghost rows; they are loaded like any row.
-#include <cstdlib>
 #include <type_traits>
 #include "vlasov_internal.cuh"
 #include "tma.cuh"
@@ -343,8 +342,7 @@ static size_t xy_smem_bytes(const Geom& G, const Species& s, int C, int xfirst) 
 static bool pick_xy_shape(const Geom& G, const Species& s, int& xb, int& C) {
     xb = 1;
     // 4 x cells per thread: 8 would halve the halo work but spills at the 128-register cap of 512 threads
-    static const char* force = getenv("VLASOV_XB");        // tuning aid: VLASOV_XB=8
-    if (G.nx % 8 == 0 && force && force[0] == '8') xb = 8; else if (G.nx % 4 == 0) xb = 4;
+    if (G.nx % 4 == 0) xb = 4;
     const int nblk = G.nx / xb;
     C = 32;
     auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && nblk * cc <= 512; };
@@ -406,7 +404,6 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
         else
         if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (v32 && G.nx == 64 && C == 32) { if (lim) launch_xy_t<4, 1, 64>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64>(tm, P, xfirst, grid, threads, smem, c->stream); }
-        else if (xb == 8) { if (lim) launch_xy_t<8, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<8, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (xb == 4) { if (lim) launch_xy_t<4, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else { if (lim) launch_xy_t<1, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
     }
