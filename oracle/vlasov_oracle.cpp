@@ -11,7 +11,7 @@
 //   f[iy_g][ix][ivx][ivy][ivz], iy_g = 0..ny+2g-1 (g ghost rows per y side), fp64.
 //   fields  E,B,J : [3][ny_g][nx];  moments: [10][ny_g][nx].
 //
-// Pins (tests/test_oracle_*.py): T1..T16 of DESIGN.md.  Parts that are pinned only by
+// Pins (tests/test_oracle_*.py): T1..T17 of DESIGN.md.  Parts that are pinned only by
 // self-consistency ("parity unpinned"): limiter under compressive velocity
 // shifts (R6/R15d), zeroth-order ghost extrapolation (R15a), isotropic target temperature (R15c),
 // ghost-row Dirichlet reuse (R16), Yee positions (R17).
