@@ -354,6 +354,16 @@ def gpu_arm(args):
             if tj.get("workload") == w.name and dom in tj.get("dram_bytes_per_launch", {}):
                 roofline["traffic"] = tj["dram_bytes_per_launch"][dom]
                 roofline["traffic_source"] = tj.get("source")
+            wi = tj.get("warp_instructions_per_launch", {}).get(dom) if tj.get("workload") == w.name else None
+            if wi and clocks and clocks.get("sm_mhz"):
+                # second roof of the same kernel: warp-instructions issued per second against 4 schedulers x SMs x
+                # the SM clock sampled during the timed region (the vy+vz kernel is issue-bound)
+                sms = torch.cuda.get_device_properties(0).multi_processor_count
+                ipeak = 4.0 * sms * clocks["sm_mhz"] * 1e6
+                iach = wi / (roofline["avg_launch_ms"] * 1e-3)
+                roofline["issue"] = {"achieved": iach / 1e9, "peak": ipeak / 1e9, "unit": "G warp-instructions/s",
+                                     "frac": iach / ipeak, "warp_instructions_per_launch": wi,
+                                     "source": tj.get("warp_instructions_source")}
     # f-sized passes of one step and species.  With FLUID sides some launches of a kind cover only ghost rows (the
     # ghost fill's velocity sweeps and edge-row moments, the x sweep of the ghost rows beside a fused stage): a kind
     # counts once per species there, and the one-direction sweeps only when no fused stage ran.
