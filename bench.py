@@ -127,7 +127,7 @@ def oracle_sample_workload(w, nx_s=16, ny_s=8):
 
 
 class OracleRun:
-    """The section-4.3 cycle composed from the oracle's own functions (no CUDA)."""
+    """State of an oracle run of a workload; the section-4.3 cycle itself is oracle.cycle (no CUDA)."""
 
     def __init__(self, ws):
         from oracle import oracle as orc
@@ -147,20 +147,12 @@ class OracleRun:
 
     def cycle(self):
         orc, w = self.orc, self.w
-        q = [sp.q for sp in self.sp]
-        J = orc.current(self.mom, q, w.fields_yee, self.wall)
-        Bavg = orc.maxwell(self.E, self.B, J, w.dx, w.dy, w.c, w.mu0, w.dt / 2, w.nsub, self.wall, want_bavg=True)
-        for s, sp in enumerate(self.sp):
-            fl = (None, None)
-            if w.bc_y_lo == inputs.BC_FLUID:
-                fl = (inputs.band_fluid_state(w, s, 0, self.step_index), inputs.band_fluid_state(w, s, 1, self.step_index))
-            err, m = orc.step(self.f[s], sp, w.nx, w.ny, w.nghost_y, w.lx, w.ly, w.dt, self.E, Bavg,
-                              fields_yee=w.fields_yee, bc_lo=w.bc_y_lo, bc_hi=w.bc_y_hi, fluid_lo=fl[0], fluid_hi=fl[1])
-            if err:
-                raise RuntimeError(f"oracle step error {err}")
-            self.mom[s] = m
-        J = orc.current(self.mom, q, w.fields_yee, self.wall)
-        orc.maxwell(self.E, self.B, J, w.dx, w.dy, w.c, w.mu0, w.dt / 2, w.nsub, self.wall)
+        fluid = None
+        if w.bc_y_lo == inputs.BC_FLUID:
+            fluid = [(inputs.band_fluid_state(w, s, 0, self.step_index), inputs.band_fluid_state(w, s, 1, self.step_index))
+                     for s in range(len(self.sp))]
+        self.mom = orc.cycle(self.f, self.sp, self.mom, self.E, self.B, w.nx, w.ny, w.nghost_y, w.lx, w.ly, w.dt, w.nsub,
+                             w.c, w.mu0, fields_yee=w.fields_yee, bc_lo=w.bc_y_lo, bc_hi=w.bc_y_hi, fluid=fluid)
         self.step_index += 1
 
 

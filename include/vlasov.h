@@ -86,7 +86,9 @@ typedef struct {
 size_t vlasov_scratch_bytes(const vlasov_config* cfg, const vlasov_species* sp /*[nspecies]*/);
 
 /* Create a context.  f_dev[s] points at species s' phase-space array (layout above).
- * Errors: EINVAL, EALIGN, ECUDA.  *out is NULL on error. */
+ * A REFLECT side needs a vy grid that is symmetric about 0 (vmin[1] == -vmax[1], R19): the wall image is built by
+ * mirroring the i_vy index.
+ * Errors: EINVAL (also: asymmetric vy grid with a REFLECT side), EALIGN, ECUDA.  *out is NULL on error. */
 int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp /*[nspecies]*/,
                 double* const* f_dev /*[nspecies], host array of device pointers*/,
                 void* scratch_dev, size_t scratch_bytes, vlasov_ctx** out);
@@ -101,7 +103,8 @@ int vlasov_set_boundary(vlasov_ctx* ctx, int species, int side, int kind, const 
  * remaps eqs. (38), (43)-(47) PAPER.md:247-295, velocity sweeps by backsubstitution eqs. (33)-(35)
  * PAPER.md:212-227 in the order vx, vy, vz.  E_dev, B_dev are the time-centred
  * fields, held fixed over the step (R11).  f is updated in the caller's buffers.
- * Errors: EINVAL; ESHIFT / EDOMAIN asynchronously (vlasov_check). */
+ * Errors: EINVAL (also: STAGE_GHOST with a FLUID side whose fluid state was never given to vlasov_set_boundary);
+ * ESHIFT / EDOMAIN asynchronously (vlasov_check). */
 int vlasov_step(vlasov_ctx* ctx, double dt, const double* E_dev, const double* B_dev, uint32_t stages);
 
 /* The same step driven from HOST buffers, the way the paper's cycle crosses the CPU/GPU border

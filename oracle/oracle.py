@@ -213,3 +213,31 @@ def step(f, sp, nx, ny, g, lx, ly, dt, E, B, fields_yee=0, limiter=1, bc_lo=BC_P
                          C.c_int(bc_lo), C.c_int(bc_hi), _d(fl), _d(fh), C.c_int(order),
                          C.c_uint(stages), _d(mom))
     return err, mom
+
+
+def cycle(f_list, sp_list, mom_list, E, B, nx, ny, g, lx, ly, dt, nsub, c, mu0, fields_yee=0, bc_lo=BC_PERIODIC,
+          bc_hi=BC_PERIODIC, fluid=None, order=ORDER_XVX, limiter=1):
+    """One time-stepping cycle of section 4.3 (Fig. 2) without the fluid step (item 4):
+      1. "the currents are calculated from the Vlasov data" (eq. 11) from the moments of f at time t (mom_list);
+      2. the fields are advanced half a step with these currents (nsub FDTD sub-steps of dt/(2 nsub), eqs. 9, 10);
+         the magnetic field is "interpolated to the time of the electric field" (PAPER.md:419);
+      3. one complete Vlasov step with the new E and that B (held fixed over the step, R11), every species;
+      5. the currents are calculated again from the new Vlasov data;
+      6. the fields are advanced another half step.
+    f_list, E, B are advanced in place ("B" stays half a sub-step ahead of "E", 8(c)-5).  fluid: None, or per species a
+    pair (fluid_lo, fluid_hi) of [5][g][nx] states for FLUID sides.  Returns the new list of moments [10][ny_g][nx]."""
+    wall = 0 if bc_lo == BC_PERIODIC else 1
+    q = [sp.q for sp in sp_list]
+    J = current(mom_list, q, fields_yee, wall)
+    Bavg = maxwell(E, B, J, lx / nx, ly / ny, c, mu0, dt / 2, nsub, wall, want_bavg=True)
+    new_mom = []
+    for s, sp in enumerate(sp_list):
+        fl = (None, None) if fluid is None else fluid[s]
+        err, m = step(f_list[s], sp, nx, ny, g, lx, ly, dt, E, Bavg, fields_yee=fields_yee, limiter=limiter,
+                      bc_lo=bc_lo, bc_hi=bc_hi, fluid_lo=fl[0], fluid_hi=fl[1], order=order)
+        if err:
+            raise RuntimeError(f"oracle step error {err}")
+        new_mom.append(m)
+    J = current(new_mom, q, fields_yee, wall)
+    maxwell(E, B, J, lx / nx, ly / ny, c, mu0, dt / 2, nsub, wall)
+    return new_mom

@@ -132,6 +132,12 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
         if (((uintptr_t)f_dev[s]) & 127) return VLASOV_EALIGN;
         if (!(sp[s].m > 0.0) || !(sp[s].f_inf > 0.0)) return VLASOV_EINVAL;
         for (int d = 0; d < 3; ++d) if (!(sp[s].vmax[d] > sp[s].vmin[d])) return VLASOV_EINVAL;
+        // a REFLECT wall builds its image by mirroring the i_vy index (R19): that is f(-vy) only on a symmetric vy grid
+        if (cfg->bc_y_lo == VLASOV_BC_REFLECT || cfg->bc_y_hi == VLASOV_BC_REFLECT) {
+            const double width = sp[s].vmax[1] - sp[s].vmin[1];
+            const double skew = sp[s].vmin[1] + sp[s].vmax[1];
+            if (!((skew < 0 ? -skew : skew) <= 1e-12 * width)) return VLASOV_EINVAL;
+        }
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) return VLASOV_ECUDA;
@@ -195,6 +201,13 @@ int vlasov_step(vlasov_ctx* c, double dt, const double* E_dev, const double* B_d
     const uint32_t vmask = c->order == VLASOV_ORDER_XVX ? VLASOV_STAGE_V : (VLASOV_STAGE_X1 | VLASOV_STAGE_X2);
     if ((stages & vmask) && (!E_dev || !B_dev)) return VLASOV_EINVAL;
     if (stages & ~(uint32_t)VLASOV_STAGE_ALL) return VLASOV_EINVAL;
+    if (stages & VLASOV_STAGE_GHOST) {
+        // a FLUID side needs its fluid state (vlasov_set_boundary) before the ghost fill can run
+        for (int s = 0; s < c->ns; ++s) {
+            if (c->G.bc_lo == VLASOV_BC_FLUID && !c->sp[s].fluid[0]) return VLASOV_EINVAL;
+            if (c->G.bc_hi == VLASOV_BC_FLUID && !c->sp[s].fluid[1]) return VLASOV_EINVAL;
+        }
+    }
     if (stages & (VLASOV_STAGE_ALL & ~VLASOV_STAGE_MOMENTS)) c->mom_valid = 0;
     for (int s = 0; s < c->ns; ++s) {
         int e = species_step(c, s, dt, E_dev, B_dev, stages);

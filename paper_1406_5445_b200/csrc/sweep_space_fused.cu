@@ -15,6 +15,9 @@
 //     previous flux per owned cell.
 // Rows -2, -1 and ny, ny+1 are the boundary rows of the y sweep (R16, R19): periodic wrap, the wall
 // image f(y_w + eta, vy) = f(y_w - eta, -vy), or FLUID ghost rows; they are loaded like any row.
+#include <mutex>
+#include <set>
+#include <tuple>
 #include <type_traits>
 #include "vlasov_internal.cuh"
 #include "tma.cuh"
@@ -316,14 +319,29 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
     }
 }
 
+// The opt-in to more than 48 KiB of dynamic shared memory is a per-device function attribute: set once per
+// (device, kernel, size), not on every launch.
+template <class K>
+static void ensure_smem_attr(K kernel, size_t smem) {
+    static std::mutex mu;
+    static std::set<std::tuple<int, const void*, size_t>> done;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const auto key = std::make_tuple(dev, (const void*)kernel, smem);
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count(key)) return;
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    done.insert(key);
+}
+
 template <int XB, int LIM, int SP, int NV = 32, int KC = xy_default_chunk(SP)>
 static void launch_xy_t(const CUtensorMap& tm, const XYParams& P, int xfirst, dim3 grid, int threads, size_t smem,
                         cudaStream_t st) {
     if (xfirst) {
-        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 1, SP, NV, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        ensure_smem_attr(sweep_xy_kernel<XB, LIM, 1, SP, NV, KC>, smem);
         sweep_xy_kernel<XB, LIM, 1, SP, NV, KC><<<grid, threads, smem, st>>>(tm, P);
     } else {
-        cudaFuncSetAttribute(sweep_xy_kernel<XB, LIM, 0, SP, NV, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        ensure_smem_attr(sweep_xy_kernel<XB, LIM, 0, SP, NV, KC>, smem);
         sweep_xy_kernel<XB, LIM, 0, SP, NV, KC><<<grid, threads, smem, st>>>(tm, P);
     }
 }

@@ -15,6 +15,9 @@
 // and the general per-face walk of march_cells.  vx: tile = all i_vx x 128 contiguous (i_vy,i_vz) cells, results
 // straight to global memory.  vy+vz fused: tile = a few contiguous i_vx planes, vy: staging -> Bf, vz: Bf -> A,
 // A -> global.  In place on f.
+#include <map>
+#include <mutex>
+#include <tuple>
 #include "vlasov_internal.cuh"
 #include "tma.cuh"
 
@@ -304,6 +307,7 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
 template <int LIM, int FAST, int LOOSE = 0, class Out>
 __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
                                             double finf, Out& out) {
+    if (a >= b) return;                              // a trailing work item beyond the end of the line: nothing to do
     double sig = fma(s1, (double)a, s0);
     constexpr int SEG = 8;
     if (FAST && b - a == SEG) {
@@ -678,22 +682,28 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     }
 }
 
-static int g_occ_x[4] = {0, 0, 0, 0}, g_occ_yz[4] = {0, 0, 0, 0};
-static size_t g_occ_x_smem[4] = {0, 0, 0, 0}, g_occ_yz_smem[4] = {0, 0, 0, 0};
 constexpr size_t V_SMEM_MAX = 200 * 1024;
 
+// Persistent grid size (resident CTAs of the device) of one kernel instantiation at one dynamic shared-memory size.
+// Function attributes and occupancy are per device: the cache is keyed by (device, kernel, smem) and guarded, so
+// several contexts on several devices (or threads) of one process each get their own answer.
 template <class K>
-static int resident_ctas(K kernel, size_t smem, int& cache, size_t& cache_smem) {
-    if (cache > 0 && cache_smem == smem) return cache;
-    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V_SMEM_MAX);
-    int per_sm = 0, dev = 0, sms = 0;
+static int resident_ctas(K kernel, size_t smem) {
+    static std::mutex mu;
+    static std::map<std::tuple<int, const void*, size_t>, int> cache;
+    int dev = 0;
     cudaGetDevice(&dev);
+    const auto key = std::make_tuple(dev, (const void*)kernel, smem);
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = cache.find(key);
+    if (it != cache.end()) return it->second;
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V_SMEM_MAX);
+    int per_sm = 0, sms = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, V_THREADS, smem);
     if (per_sm < 1) per_sm = 1;
-    cache = per_sm * sms;
-    cache_smem = smem;
-    return cache;
+    cache[key] = per_sm * sms;
+    return per_sm * sms;
 }
 
 int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost) {
@@ -721,7 +731,6 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         void (*k)(VParams) = lim ? vsweep_x_kernel<1, 0> : vsweep_x_kernel<0, 0>;
         if (spec == 16) k = lim ? vsweep_x_kernel<1, 16> : vsweep_x_kernel<0, 16>;
         if (spec == 32) k = lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>;
-        const int cube32 = spec ? 1 : 0;
         const int tspec = (cn == 16 || cn == 24 || cn == 32 || cn == 40 || cn == 48) ? cn : 0;
         if (tspec && !ghost && (long)c->G.nyg * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
             // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]; its own tile shape
@@ -736,14 +745,11 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (tspec == 40) kt = lim ? vsweep_x_tma_kernel<1, 40> : vsweep_x_tma_kernel<0, 40>;
             if (tspec == 48) kt = lim ? vsweep_x_tma_kernel<1, 48> : vsweep_x_tma_kernel<0, 48>;
             const size_t smem_t = (size_t)(3 * V_PAD + 2 * tspec) * 128 * 8 + 16;
-            static int occ_t[16] = {0};
-            static size_t occ_t_smem[16] = {0};
-            const int gi = lim + 2 * (tspec / 8);
-            const int grid = min(P.ntot, resident_ctas(kt, smem_t, occ_t[gi], occ_t_smem[gi]));
+            const int grid = min(P.ntot, resident_ctas(kt, smem_t));
             Launch L(c, K_VSWEEP_X);
             kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);
         } else {
-            const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_x[lim + 2 * cube32], g_occ_x_smem[lim + 2 * cube32]));
+            const int grid = min(P.ntot, resident_ctas(k, smem));
             Launch L(c, K_VSWEEP_X);
             k<<<grid, V_THREADS, smem, c->stream>>>(P);
         }
@@ -772,7 +778,6 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 32) k = lim ? vsweep_yz_kernel<1, 32> : vsweep_yz_kernel<0, 32>;
         if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
         if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
-        const int sq32 = spec ? 1 : 0;
         if (spec && spec != 48 && (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1] < 2147483647L) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
             // TMA-staged variant: f as a matrix [cells * nv0 * nv1][nv2], one box {nv2, nv1} per plane
             CUtensorMap tm;
@@ -785,14 +790,11 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
             const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8;
             if (smem_t > V_SMEM_MAX) return VLASOV_EINVAL;
-            static int occ_t[16] = {0};
-            static size_t occ_t_smem[16] = {0};
-            const int gi = lim + 2 * (spec / 8);
-            const int grid = min(P.ntot, resident_ctas(kt, smem_t, occ_t[gi], occ_t_smem[gi]));
+            const int grid = min(P.ntot, resident_ctas(kt, smem_t));
             Launch L(c, K_VSWEEP_YZ);
             kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);
         } else {
-            const int grid = min(P.ntot, resident_ctas(k, smem, g_occ_yz[lim + 2 * sq32], g_occ_yz_smem[lim + 2 * sq32]));
+            const int grid = min(P.ntot, resident_ctas(k, smem));
             Launch L(c, K_VSWEEP_YZ);
             k<<<grid, V_THREADS, smem, c->stream>>>(P);
         }

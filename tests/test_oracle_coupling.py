@@ -221,6 +221,57 @@ def test_R17_yee_positions_linear_fields_interpolate_exactly(orc):
     assert Ec[1] == 0.5 * ((nx - 1) + 0)
 
 
+@pytest.mark.parametrize("ix", [0, 2, 5])
+def test_R17_yee_gather_at_the_pec_wall_rows(orc, ix):
+    """wall = 1 (R17): the walls are the node rows j = 0 and j = nyg; E_x, E_z and B_y vanish there.
+    The array holds rows 0 .. nyg-1, so the gather of the TOP row of cells reads "row nyg" as the wall value 0, and
+    the gather of the BOTTOM row reads row 0 as stored.  Pin: fields that are linear in y and vanish on the top wall
+    are interpolated exactly to the centres of the top row; with the periodic reading (wall = 0) the same call wraps
+    to row 0.  Mutants of orc_field_at_cell that fail: "up" left at 1 with a wall (row 0 read as the wall), "up"
+    applied to a half-row component (E_y, B_x), jp not wrapped."""
+    nx, nyg, dx, dy = 6, 5, 0.5, 0.25
+    top = nyg * dy
+    xi, yj = np.arange(nx) * dx, np.arange(nyg) * dy
+    X, Y = np.meshgrid(xi, yj, indexing="xy")
+    W = lambda x, y, k: (1.0 + 0.5 * k) * (top - y)                 # vanishes on the top wall
+    F = lambda x, y, k: 2.0 + k + 0.3 * y                           # half-row components: no wall value involved
+    E = np.stack([W(X + dx / 2, Y, 0), F(X, Y + dy / 2, 1), W(X, Y, 2)])
+    B = np.stack([F(X, Y + dy / 2, 3), W(X + dx / 2, Y, 4), F(X + dx / 2, Y + dy / 2, 5)])
+    j = nyg - 1
+    xc, yc = (ix + 0.5) * dx, (j + 0.5) * dy
+    Ec, Bc = orc.field_at_cell(E, B, 1, 1, ix, j)
+    assert np.allclose(Ec, [W(xc, yc, 0), F(xc, yc, 1), W(xc, yc, 2)], rtol=1e-14)
+    assert np.allclose(Bc, [F(xc, yc, 3), W(xc, yc, 4), F(xc, yc, 5)], rtol=1e-14)
+    # periodic reading of the same arrays: row nyg is row 0, where W = (1 + k/2) top
+    Ep, Bp = orc.field_at_cell(E, B, 1, 0, ix, j)
+    assert np.isclose(Ep[0], 0.5 * (W(xc, j * dy, 0) + W(xc, 0.0, 0)), rtol=1e-14) and Ep[0] > 2 * Ec[0]
+    assert np.isclose(Ep[2], 0.5 * (W(xc, j * dy, 2) + W(xc, 0.0, 2)), rtol=1e-14)
+    assert np.isclose(Bp[1], 0.5 * (W(xc, j * dy, 4) + W(xc, 0.0, 4)), rtol=1e-14)
+    assert Ep[1] == Ec[1] and Bp[0] == Bc[0] and Bp[2] == Bc[2]
+    # bottom row of cells: row 0 is read as stored (the Maxwell solver keeps the wall values at zero there), so
+    # fields linear in y interpolate exactly whatever the wall flag
+    for wall in (0, 1):
+        E0, B0 = orc.field_at_cell(E, B, 1, wall, ix, 0)
+        assert np.allclose(E0, [W(xc, dy / 2, 0), F(xc, dy / 2, 1), W(xc, dy / 2, 2)], rtol=1e-14)
+        assert np.allclose(B0, [F(xc, dy / 2, 3), W(xc, dy / 2, 4), F(xc, dy / 2, 5)], rtol=1e-14)
+
+
+def test_eq11_current_on_the_yee_grid_wraps_or_hits_the_wall_at_row_0(orc):
+    """eq. 11 on the E positions of R17 at row 0: periodic (wall = 0) averages rows nyg-1 and 0; with a PEC wall the
+    tangential components J_x, J_z of the wall row are not used (E_x = E_z = 0 there) and are stored as 0.  J_y sits
+    at half rows and is not affected.  Mutants that fail: the wall flag ignored, wrap to the wrong row."""
+    nx, nyg = 4, 5
+    m1 = np.zeros((10, nyg, nx))
+    row = np.arange(nyg, dtype=float)[:, None] + 0 * np.arange(nx)[None, :]
+    m1[1] = 1.0 + row; m1[2] = 10.0 + row; m1[3] = 100.0 + 2 * row
+    Jp = orc.current([m1], [2.0], fields_yee=1, wall=0)
+    assert np.allclose(Jp[0, 0], 2.0 * 0.5 * ((1.0 + nyg - 1) + 1.0)) and np.allclose(Jp[2, 0], 2.0 * 0.5 * ((100.0 + 2 * (nyg - 1)) + 100.0))
+    assert np.allclose(Jp[1, 0], 2.0 * 10.0)
+    Jw = orc.current([m1], [2.0], fields_yee=1, wall=1)
+    assert not Jw[0, 0].any() and not Jw[2, 0].any() and np.allclose(Jw[1, 0], 20.0)
+    assert np.array_equal(Jw[:, 1:], Jp[:, 1:])
+
+
 def test_eq11_current_from_moments(orc):
     nx, nyg = 5, 4
     rng = np.random.default_rng(16)

@@ -13,7 +13,10 @@ def _species(orc, nv, vmin, vmax, q=-1.0, m=1.0, finf=1.0):
     return orc.Species(q, m, nv, vmin, vmax, finf)
 
 
-def test_T10_free_streaming_is_exact_translation(orc):
+@pytest.mark.parametrize("order", [0, 1])
+def test_T10_free_streaming_is_exact_translation(orc, order):
+    """order = 1 (VXV): the one spatial step of the cycle takes the FULL dt (mutant "dts = dt/2 in the VXV
+    branch" translates by half the distance and fails here)."""
     # v centres -3,-1,1,3 (x), -2.5,-1.5,...(y scaled so shifts are integers): dt/(2 dx) = 1, dt/(2 dy) = 2
     nx, ny = 12, 10
     nv = (4, 4, 2)
@@ -23,7 +26,7 @@ def test_T10_free_streaming_is_exact_translation(orc):
     f0 = rng.random((ny, nx) + nv)
     f = f0.copy()
     Z = np.zeros((3, ny, nx))
-    err, _ = orc.step(f, sp, nx, ny, 0, lx, ly, dt, Z, Z, limiter=1)
+    err, _ = orc.step(f, sp, nx, ny, 0, lx, ly, dt, Z, Z, limiter=1, order=order)
     assert err == 0
     vx = sp.vmin[0] + (np.arange(nv[0]) + 0.5) * 2.0
     vy = sp.vmin[1] + (np.arange(nv[1]) + 0.5) * 0.5
@@ -36,8 +39,9 @@ def test_T10_free_streaming_is_exact_translation(orc):
             assert np.abs(f[:, :, a, b, :] - want).max() <= 1e-14, (a, b)
 
 
+@pytest.mark.parametrize("order", [0, 1])
 @pytest.mark.parametrize("bc", ["periodic", "reflect"])
-def test_T11_uniform_maxwellian_is_invariant_bit_for_bit(orc, bc):
+def test_T11_uniform_maxwellian_is_invariant_bit_for_bit(orc, bc, order):
     nx, ny, nv = 6, 5, (8, 8, 8)
     sp = _species(orc, nv, (-6.0,) * 3, (6.0,) * 3)
     c = sp.vmin[0] + (np.arange(8) + 0.5) * 1.5
@@ -48,7 +52,7 @@ def test_T11_uniform_maxwellian_is_invariant_bit_for_bit(orc, bc):
     f = f0.copy()
     Z = np.zeros((3, ny, nx))
     b = orc.BC_PERIODIC if bc == "periodic" else orc.BC_REFLECT
-    err, mom = orc.step(f, sp, nx, ny, 0, 3.0, 2.0, 0.37, Z, Z, bc_lo=b, bc_hi=b)
+    err, mom = orc.step(f, sp, nx, ny, 0, 3.0, 2.0, 0.37, Z, Z, bc_lo=b, bc_hi=b, order=order)
     assert err == 0
     assert np.array_equal(f, f0)
     assert np.ptp(mom[0]) == 0.0
@@ -64,8 +68,9 @@ def _smooth_state(nx, ny, nv, sp, rng):
     return prof[:, :, None, None, None] * M[None, None]
 
 
+@pytest.mark.parametrize("order", [0, 1])
 @pytest.mark.parametrize("bc", ["periodic", "reflect"])
-def test_T5_full_step_conserves_mass_to_roundoff(orc, bc):
+def test_T5_full_step_conserves_mass_to_roundoff(orc, bc, order):
     nx, ny, nv = 8, 6, (8, 8, 8)
     sp = _species(orc, nv, (-5.0,) * 3, (5.0,) * 3, q=-1.0, m=0.5)
     rng = np.random.default_rng(5)
@@ -76,7 +81,7 @@ def test_T5_full_step_conserves_mass_to_roundoff(orc, bc):
     b = orc.BC_PERIODIC if bc == "periodic" else orc.BC_REFLECT
     m0 = f.sum()
     for _ in range(3):
-        err, mom = orc.step(f, sp, nx, ny, 0, 4.0, 3.0, 0.2, E, B, bc_lo=b, bc_hi=b)
+        err, mom = orc.step(f, sp, nx, ny, 0, 4.0, 3.0, 0.2, E, B, bc_lo=b, bc_hi=b, order=order)
         assert err == 0
     assert abs(f.sum() - m0) / m0 <= 1e-14
     dv3 = (10.0 / 8) ** 3
@@ -145,7 +150,7 @@ def test_x_sweep_covers_ghost_rows(orc):
         assert not np.array_equal(f[r], f0[r])
 
 
-def _strang_run(orc, nsteps, T=0.8):
+def _strang_run(orc, nsteps, T=0.8, order=0):
     """1D1V (x, vx) smooth problem with a prescribed travelling-wave E_x(x, t); E passed at mid-step (R11)."""
     nx, nvx = 64, 128
     nv = (nvx, 1, 1)
@@ -159,16 +164,25 @@ def _strang_run(orc, nsteps, T=0.8):
     for n in range(nsteps):
         E = Z.copy()
         E[0, 0] = 1.5 * np.sin(x - 0.7 * (n + 0.5) * dt)
-        err, _ = orc.step(f, sp, nx, 1, 0, lx, 1.0, dt, E, Z, limiter=0, want_moments=False)
+        err, _ = orc.step(f, sp, nx, 1, 0, lx, 1.0, dt, E, Z, limiter=0, want_moments=False, order=order)
         assert err == 0
     return f
 
 
-def test_T16_strang_splitting_is_second_order(orc):
-    ref = _strang_run(orc, 64)
-    e = [np.abs(_strang_run(orc, n) - ref).max() for n in (2, 4, 8)]
+@pytest.mark.parametrize("order", [0, 1])
+def test_T16_strang_splitting_is_second_order(orc, order):
+    """Both orders of R2 are second order (eq. 22; PAPER.md:420 for VXV = order 1), and they solve the
+    same equation: the fine VXV run converges to the fine XVX run.  Mutants of the VXV branch that fail here: a
+    velocity half taking dt instead of dt/2 (O(1) error against the XVX reference), the second velocity half dropped
+    (first order), the spatial step taking dt/2."""
+    ref = _strang_run(orc, 64, order=order)
+    e = [np.abs(_strang_run(orc, n, order=order) - ref).max() for n in (2, 4, 8)]
     r1, r2 = e[0] / e[1], e[1] / e[2]
     assert 3.3 < r1 < 5.0 and 3.3 < r2 < 5.0, (e, r1, r2)
+    if order == 1:
+        ref_xvx = _strang_run(orc, 64, order=0)
+        # two second-order schemes at dt = T/64: their difference is far below the dt = T/8 error of either
+        assert np.abs(ref - ref_xvx).max() < 0.05 * e[2], (np.abs(ref - ref_xvx).max(), e)
 
 
 def _landau_run(orc, steps):
@@ -197,6 +211,44 @@ def _landau_run(orc, steps):
         err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, Z, Z, stages=orc.STAGE_X2)
         assert err == 0
         t.append((n + 0.5) * w.dt)
+        W.append(0.5 * np.sum(Ex ** 2) * w.dx)
+    return np.array(t), np.array(W), abs(f.sum() - m0) / m0
+
+
+def _landau_run_vxv(orc, steps):
+    """Config 1 under the order of the paper's coupled cycle (reading R2): "half a step in velocity space,
+    a full step in physical space and half a step in velocity space".  The density does not change during a velocity
+    step, so the field computed after the spatial step is E^{n+1}: it drives the second velocity half of step n and
+    the first velocity half of step n+1 (time-centred between the two halves it separates)."""
+    w = inputs.landau_workload(steps=steps)
+    spec = w.species[0]
+    f = inputs.landau_f(w)
+    sp = orc.Species(spec.q, spec.m, spec.nv, spec.vmin, spec.vmax, spec.f_inf)
+    nx, ny = w.nx, w.ny
+    k = 2 * np.pi * np.fft.fftfreq(nx, d=w.dx)
+    Z = np.zeros((3, ny, nx))
+    m0 = f.sum()
+
+    def poisson():
+        ne = orc.moments(f, sp, nx, ny, 0)[0].mean(axis=0)
+        rho_hat = np.fft.fft(1.0 - ne)
+        Eh = np.zeros(nx, dtype=complex)
+        Eh[1:] = rho_hat[1:] / (1j * k[1:])
+        return np.fft.ifft(Eh).real
+
+    Ex = poisson()
+    t, W = [], []
+    for n in range(steps):
+        E = Z.copy(); E[0] = Ex[None, :]
+        err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, E, Z, order=orc.ORDER_VXV, stages=orc.STAGE_X1)
+        assert err == 0
+        err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, Z, Z, order=orc.ORDER_VXV, stages=orc.STAGE_V)
+        assert err == 0
+        Ex = poisson()
+        E = Z.copy(); E[0] = Ex[None, :]
+        err, _ = orc.step(f, sp, nx, ny, 0, w.lx, w.ly, w.dt, E, Z, order=orc.ORDER_VXV, stages=orc.STAGE_X2)
+        assert err == 0
+        t.append((n + 1) * w.dt)
         W.append(0.5 * np.sum(Ex ** 2) * w.dx)
     return np.array(t), np.array(W), abs(f.sum() - m0) / m0
 
@@ -232,3 +284,21 @@ def test_T12_landau_damping_rate(orc):
     assert first.sum() == 2
     g100 = 0.5 * (wp[first][1] - wp[first][0]) / (tp[first][1] - tp[first][0])
     assert abs(g100 + 0.1533) <= 0.013, g100
+
+
+@pytest.mark.slow
+def test_T12_landau_damping_rate_vxv(orc):
+    """The same textbook rate under ORDER_VXV, with the stage mask of that order: X1 = first velocity
+    half, V = the full spatial step, X2 = second velocity half.  Mutants of the oracle's VXV branch that fail here: the
+    XVX sequence taken for order = 1 (the harness then kicks with E during "spatial" stages: no damping at the right
+    rate), a velocity half with dt instead of dt/2 (plasma frequency off by sqrt(2): omega gate), the spatial step
+    with dt/2 (omega gate), a dropped half."""
+    t, W, drift = _landau_run_vxv(orc, 400)
+    assert drift <= 1e-13
+    tp, wp = _peaks(t, W)
+    sel = (tp > 2.0) & (tp < 18.5)
+    assert sel.sum() >= 7
+    gamma = np.polyfit(tp[sel], wp[sel], 1)[0] / 2
+    omega = np.pi / np.mean(np.diff(tp[sel]))
+    assert abs(gamma + 0.1533) <= 0.004, gamma
+    assert abs(omega - 1.4157) <= 0.005, omega
