@@ -50,6 +50,17 @@ def make_workload(name):
     raise SystemExit(f"unknown workload {name}")
 
 
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for ln in fh:
+                if ln.lower().startswith("model name"):
+                    return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -236,7 +247,7 @@ def gpu_arm(args):
     fluid = None
     if w.bc_y_lo == inputs.BC_FLUID:
         # seeded 5-moment states, redrawn per step from the step index (config 4); resident before timing
-        nstate = args.warmup + args.steps + 2 * args.steps + 8
+        nstate = args.warmup + (args.reps + 2) * args.steps + 8
         fluid = [[[torch.from_numpy(inputs.band_fluid_state(w, s, side, k)).to(device) for side in (0, 1)]
                   for s in range(ns)] for k in range(nstate)]
     step_no = [0]
@@ -256,32 +267,47 @@ def gpu_arm(args):
             torch.cuda.synchronize()
 
     # ---- device-resident leg: `value` -------------------------------------------------------
+    # Timed with the library's per-launch event pairs OFF.  REPS repetitions of the timed block (each EXACTLY
+    # args.steps cycles between barrier + synchronize); the reported time is the median.
     for _ in range(args.warmup):
         set_fluid()
         ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
     ctx.vlasov_check()
+    ctx.vlasov_timing_enable(False)
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    rep_ms, launches = [], 0
+    t_wall0 = time.time()
+    for _ in range(max(1, args.reps)):
+        barrier()
+        l0 = ctx.launch_count()
+        ev0.record(stream)
+        for _ in range(args.steps):
+            set_fluid()
+            ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+        ev1.record(stream)
+        barrier()
+        launches = ctx.launch_count() - l0
+        rep_ms.append(max_over_ranks(ev0.elapsed_time(ev1), dist, device))
+    t_wall1 = time.time()
+    ctx.vlasov_check()
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms = float(np.median(rep_ms))
+    cells = w.interior_cells
+    value = whole_job_value(cells, args.steps, ms, world)
+
+    # ---- the same number of steps again with an event pair around every launch: the per-kernel table ----
     ctx.vlasov_timing_enable(True)
     barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
-    l0 = ctx.launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_wall0 = time.time()
     ev0.record(stream)
     for _ in range(args.steps):
         set_fluid()
         ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
     ev1.record(stream)
     barrier()
-    t_wall1 = time.time()
-    ctx.vlasov_check()
-    launches = ctx.launch_count() - l0
-    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
-    ms = ev0.elapsed_time(ev1)
+    ms_instr = ev0.elapsed_time(ev1)
     per_kind = ctx.vlasov_timing_read()
     ctx.vlasov_timing_enable(False)
-    ms = max_over_ranks(ms, dist, device)
-    cells = w.interior_cells
-    value = whole_job_value(cells, args.steps, ms, world)
 
     # ---- end-to-end leg: HOST buffers through the C ABI (vlasov_cycle_host) -----------------
     ncell = w.ny_g * w.nx
@@ -316,6 +342,7 @@ def gpu_arm(args):
     # ---- roofline of the dominant kernel (CUDA-event pairs around every launch, timed region) ----
     peak, peak_src = peaks()
     cells_all = sum(w.ny_g * w.nx * s.ncell_v for s in w.species) / ns      # ghost-inclusive, per species launch
+    cells_int = cells / ns                                                     # interior rows only
     kinds = {}
     tot_ms = sum(v[0] for v in per_kind.values())
     for k, (kms, cnt) in per_kind.items():
@@ -323,21 +350,21 @@ def gpu_arm(args):
             continue
         ent = {"ms_per_step": kms / args.steps, "launches_per_step": cnt / args.steps, "share": kms / tot_ms}
         if k in BYTES_PER_CELL:
-            # vsweep/moments launches that only cover ghost rows or one edge row (ghost fill) are small; the
-            # average below is over launches of this kind, bytes are summed over what each launch covers
-            # (with FLUID sides some launches of a kind cover only ghost rows: no per-launch figure then)
-            bytes_total = BYTES_PER_CELL[k] * cells_all * cnt if fluid is None else None
-            if bytes_total is not None:
-                ent["gbs"] = bytes_total / (kms * 1e-3) / 1e9
-                ent["frac_of_peak"] = ent["gbs"] / peak
+            # the fused spatial stages cover the interior rows (ghost rows are Dirichlet data, R16); the velocity sweeps and
+            # the moments pass cover every row.  Ghost-fill launches have their own kinds (ghost_*) and are not mixed in.
+            ncells = cells_int if k in ("sweep_xy", "sweep_yx") else cells_all
+            ent["gbs"] = BYTES_PER_CELL[k] * ncells * cnt / (kms * 1e-3) / 1e9
+            ent["frac_of_peak"] = ent["gbs"] / peak
+            ent["cells_per_launch"] = ncells
         kinds[k] = ent
+    ghost_ms = sum(v["ms_per_step"] for k, v in kinds.items() if k.startswith("ghost_"))
     dom = max((k for k in kinds if "gbs" in kinds[k]), key=lambda k: kinds[k]["share"], default=None)
     roofline = None
     if dom is not None:
         d = kinds[dom]
         roofline = {"kernel": dom, "bound": "hbm", "achieved": d["gbs"], "peak": peak, "unit": "GB/s",
                     "frac": d["gbs"] / peak, "traffic": None, "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": BYTES_PER_CELL[dom] * cells_all,
+                    "algorithmic_bytes_per_launch": BYTES_PER_CELL[dom] * d["cells_per_launch"],
                     "avg_launch_ms": d["ms_per_step"] / d["launches_per_step"], "share_of_step": d["share"]}
         tr = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tr):
@@ -356,28 +383,32 @@ def gpu_arm(args):
                 roofline["issue"] = {"achieved": iach / 1e9, "peak": ipeak / 1e9, "unit": "G warp-instructions/s",
                                      "frac": iach / ipeak, "warp_instructions_per_launch": wi,
                                      "source": tj.get("warp_instructions_source")}
-    # f-sized passes of one step and species.  With FLUID sides some launches of a kind cover only ghost rows (the
-    # ghost fill's velocity sweeps and edge-row moments, the x sweep of the ghost rows beside a fused stage): a kind
-    # counts once per species there, and the one-direction sweeps only when no fused stage ran.
+    # f-sized passes of one step and species (the ghost_* kinds are overhead of the FLUID border, not passes); the
+    # one-direction sweeps count only when no fused stage ran.
     fused = any(k in kinds for k in ("sweep_xy", "sweep_yx"))
 
     def full_passes(k, v):
         n = v["launches_per_step"] / ns
         if k in ("sweep_x", "sweep_y"):
             return 0.0 if fused else n
-        return min(n, 1.0) if fluid is not None else n
+        return n
 
-    pass_bytes = sum(BYTES_PER_CELL[k] * full_passes(k, v) for k, v in kinds.items() if k in BYTES_PER_CELL)
+    step_bytes = sum(BYTES_PER_CELL[k] * v["cells_per_launch"] * full_passes(k, v) * ns
+                     for k, v in kinds.items() if k in BYTES_PER_CELL)
+    pass_bytes = step_bytes / cells           # per interior cell-update
 
     # ---- the oracle timed beside it (reported baseline only) --------------------------------
     cpu = None
     if not args.no_cpu_baseline:
         v, _, cores, sample, _ = oracle_leg(make_workload(args.workload), steps=50, warmup=1, budget_s=args.cpu_budget)
-        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle", "sample": sample}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "timing": {"what": "median of the repetitions; each repetition times exactly `steps` cycles, per-launch event pairs off",
+                   "repetitions": len(rep_ms), "ms_per_step_each": [m / args.steps for m in rep_ms],
+                   "ms_per_step_with_per_launch_events": ms_instr / args.steps},
         "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise, DESIGN.md 'Input recipe')",
         "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nghost_y": w.nghost_y,
                    "nv": list(w.species[0].nv), "species": ns, "dt": w.dt, "maxwell_nsub": w.nsub,
@@ -390,11 +421,15 @@ def gpu_arm(args):
         "gpu_launches": launches,
         "roofline": roofline,
         "step_hbm": {"algorithmic_bytes_per_cell_update": pass_bytes,
-                     "achieved_gbs": pass_bytes * cells_all * ns * args.steps / (ms * 1e-3) / 1e9,
-                     "note": "sum over the step's f-sized passes (ghost-inclusive cells) / step time"},
+                     "achieved_gbs": step_bytes * args.steps / (ms * 1e-3) / 1e9,
+                     "note": "sum over the step's f-sized passes (cells each pass covers; ghost_* launches not credited) / step time"},
         "kernels": kinds,
         "cpu_baseline": cpu,
     }
+    if fluid is not None:
+        # what the FLUID border costs (ghost fill: edge moments + table + three remaps of the ghost
+        # rows; x sweeps of the ghost rows), as a share of the per-launch-timed step
+        out["ghost_fill_share_of_step"] = (ghost_ms + kinds.get("ghost_table", {}).get("ms_per_step", 0.0)) / (tot_ms / args.steps)
     out["step_hbm"]["frac_of_peak"] = out["step_hbm"]["achieved_gbs"] / peak
     # SURVEY.md 8(d) reporting rule: the same figure against the nominal 8 TB/s, and the "useful" fraction that
     # credits only the 48 B per cell-update of the 3-pass Strang floor (x/2 y/2, V, y/2 x/2 each once through HBM)
@@ -416,7 +451,7 @@ def reference_arm(args):
            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise)",
            "config": {"workload": w.name, "sample": sample},
-           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle", "sample": sample},
            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out))
@@ -427,6 +462,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed block of --steps cycles (median reported)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="gem128")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -164,7 +164,11 @@ int vlasov_cycle_host(vlasov_ctx* ctx, double dt, int nsub, double* E_host, doub
 enum {
     VLASOV_KIND_SWEEP_X = 0, VLASOV_KIND_SWEEP_Y, VLASOV_KIND_TABLE, VLASOV_KIND_VSWEEP_X, VLASOV_KIND_VSWEEP_YZ,
     VLASOV_KIND_MOMENTS, VLASOV_KIND_GHOST_TABLE, VLASOV_KIND_CURRENT, VLASOV_KIND_MAXWELL, VLASOV_KIND_SWEEP_XY /* fused x/2 y/2 */,
-    VLASOV_KIND_SWEEP_YX /* fused y/2 x/2 */, VLASOV_KIND_COUNT
+    VLASOV_KIND_SWEEP_YX /* fused y/2 x/2 */,
+    /* launches that only exist because a side is FLUID (config 4's "ghost-fill share of step time"): the ghost fill's
+     * velocity remaps and edge-row moments (section 4.2), and the x sweeps of the ghost rows beside a fused stage */
+    VLASOV_KIND_GHOST_VSWEEP_X, VLASOV_KIND_GHOST_VSWEEP_YZ, VLASOV_KIND_GHOST_MOMENTS, VLASOV_KIND_GHOST_SWEEP_X,
+    VLASOV_KIND_COUNT
 };
 int vlasov_timing_enable(vlasov_ctx* ctx, int on);
 int vlasov_timing_read(vlasov_ctx* ctx, double* ms_by_kind, int64_t* count_by_kind, int nkinds);

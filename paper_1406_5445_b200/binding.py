@@ -8,7 +8,8 @@ import ctypes as C
 import os
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libvlasov_b200.so")
+# VLASOV_B200_LIB: another build of the same library (A/B measurements of kernel variants); default: the in-tree build
+LIB_PATH = os.environ.get("VLASOV_B200_LIB") or os.path.join(HERE, "libvlasov_b200.so")
 
 OK, EINVAL, EALIGN, ESHIFT, EDOMAIN, ECUDA = 0, -1, -2, -3, -4, -5
 BC_PERIODIC, BC_REFLECT, BC_FLUID = 0, 1, 2
@@ -20,7 +21,8 @@ EXPORTS = ["vlasov_scratch_bytes", "vlasov_init", "vlasov_set_boundary", "vlasov
            "vlasov_launch_count", "vlasov_free", "vlasov_strerror", "vlasov_cycle", "vlasov_cycle_host",
            "vlasov_timing_enable", "vlasov_timing_read", "vlasov_fluid_boundary_mark", "vlasov_fluid_boundary"]
 OPT_FUSE_XY = 1
-KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy", "sweep_yx"]
+KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy", "sweep_yx",
+         "ghost_vsweep_x", "ghost_vsweep_yz", "ghost_moments", "ghost_sweep_x"]
 
 
 class vlasov_species(C.Structure):

@@ -45,8 +45,12 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
     const Geom& G = c->G;
     int e;
     if (stages & VLASOV_STAGE_GHOST) {
-        if (G.bc_lo == VLASOV_BC_FLUID) { e = launch_ghost_fill(c, s, s.f, 0); if (e) return e; }
-        if (G.bc_hi == VLASOV_BC_FLUID) { e = launch_ghost_fill(c, s, s.f, 1); if (e) return e; }
+        c->ghost_tag = 1;
+        e = VLASOV_OK;
+        if (G.bc_lo == VLASOV_BC_FLUID) e = launch_ghost_fill(c, s, s.f, 0);
+        if (!e && G.bc_hi == VLASOV_BC_FLUID) e = launch_ghost_fill(c, s, s.f, 1);
+        c->ghost_tag = 0;
+        if (e) return e;
     }
     // cur: where this species' f lives right now.  The general spatial stage is f -> pong -> f; the fused
     // stage is ONE pass cur -> other, so the buffers swap roles; an odd number of fused stages in one call
@@ -58,8 +62,11 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         if (c->fuse_xy && fused_xy_applicable(c, s, dts)) {
             r = launch_sweep_xy(c, s, cur, other, dts, x_first ? 1 : 0); if (r) return r;
             if (G.g > 0) {      // x sweeps update ghost rows too, y sweeps never do (R16)
-                r = launch_sweep_x_rows(c, s, cur, other, dts, 0, G.g); if (r) return r;
-                r = launch_sweep_x_rows(c, s, cur, other, dts, G.g + G.ny, G.g); if (r) return r;
+                c->ghost_tag = 1;
+                r = launch_sweep_x_rows(c, s, cur, other, dts, 0, G.g);
+                if (!r) r = launch_sweep_x_rows(c, s, cur, other, dts, G.g + G.ny, G.g);
+                c->ghost_tag = 0;
+                if (r) return r;
             }
             cur = other;
             return VLASOV_OK;
@@ -176,7 +183,7 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     c->Jbuf = (double*)(base + C.jbuf);
     c->Bavg = (double*)(base + C.bavg);
     c->errflag = (int*)(base + C.err);
-    c->timing = 0; c->nrec = 0; c->ev0 = c->ev1 = nullptr; c->rec_kind = nullptr;
+    c->timing = 0; c->ghost_tag = 0; c->nrec = 0; c->ev0 = c->ev1 = nullptr; c->rec_kind = nullptr;
     c->mom_valid = 0;
     c->fuse_xy = 1;
     c->launches = 0;

@@ -54,7 +54,9 @@ struct Weights {
 // Does the slope pair (dp, dm) of a cell with value f0 possibly need limiting?  High-word test of
 // vlasov_internal.cuh (conservative).  Returns a word whose sign bit is set if so.
 __device__ __forceinline__ int need_bits(double f0, double dp, double dm, double finf) {
-    const int hb = min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000;
+    // f0 < 0 or f0 > f_inf (round-off leaves -1e-17 behind): the high word is hugely negative, and the difference
+    // below would wrap around; max(., 0) keeps the answer "yes" there
+    const int hb = max(min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000, 0);
     const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
     return (hb - 1) - max(hp, hm);
 }

@@ -165,6 +165,18 @@ __device__ __forceinline__ double face_flux_pad(unsigned L, int st8, int N, int 
 // Zero cells on either side of every line of a tile (f = 0 outside the box, R7): the general walk clamps the foot to
 // [-2, N+1] and reads its two neighbours, the register-window walk reads cells -2 .. N+1.
 constexpr int V_PAD = 3;
+// Faces per limiter vote of the register-window walk (march_seg_small).  The vx kernel has registers to spare (2 CTAs
+// per SM): 3 faces per vote give it three independent flux evaluations between votes.  The vy+vz kernel runs 3 CTAs
+// per SM at 80 registers, where batches spill: one face per vote (measured, profiles/README.md).
+#ifndef VL_X_BATCH
+#define VL_X_BATCH 3
+#endif
+#ifndef VL_YZ_BATCH
+#define VL_YZ_BATCH 1
+#endif
+#ifndef VL_YZ_MINB
+#define VL_YZ_MINB 3
+#endif
 
 struct OutShared {       // cells of a line in shared memory: cell0 = byte address of cell a
     unsigned a; int st8;
@@ -182,7 +194,9 @@ struct OutGlobal {       // cells of a line in global memory (streaming store)
 // Does the slope pair (dp, dm) of a cell with value f0 possibly need limiting?  High-word test of slopes_fast
 // (conservative).  The sign bit of the result is set if so.
 __device__ __forceinline__ int need_bits(double f0, double dp, double dm, double finf) {
-    const int hb = min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000;
+    // f0 < 0 or f0 > f_inf (round-off leaves -1e-17 behind): the high word is hugely negative, and the difference
+    // below would wrap around; max(., 0) keeps the answer "yes" there
+    const int hb = max(min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000, 0);
     const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
     return (hb - 1) - max(hp, hm);
 }
@@ -192,7 +206,7 @@ __device__ __forceinline__ int need_bits(double f0, double dp, double dm, double
 // (eq. 47 = eq. 46 on the mirrored line), and face m of the walk takes (q[m], q[m+1], q[m+2]).  About a
 // quarter of the instructions of the general walk below.
 //   walk position i <-> cell a-2+i (sigma >= 0) | a+SEG+1-i (sigma < 0);  face m <-> face a+m | a+SEG-m.
-template <int SEG, int LIM, int FULL, class Out>
+template <int SEG, int LIM, int FULL, int NB, class Out>
 __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
                                                 double s1, double finf, Out out) {
     const bool pos = !(sig_a < 0.0 || sig_b < 0.0);      // the caller made sure the two do not disagree
@@ -210,19 +224,60 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
     if (!pos) { out.skip(SEG - 1); }
     out.step(dir);
     double Gp = 0.0;
+    // NB faces at a time: ONE limiter vote per batch (all lanes sit on the same faces), so that the NB flux
+    // evaluations are independent instruction streams between the votes
 #pragma unroll
-    for (int m = 0; m <= SEG; ++m) {
-        double sp, sm;
-        slopes_fast<LIM, FULL>(q[m], q[m + 1], q[m + 2], finf, sp, sm);     // all lanes sit on the same face: one vote per face
-        const double bq = fabs(sig);
-        const double b2 = bq * bq;
-        const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
-        const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
-        double G = bq * fma(c1, sp, fma(c2, sm, q[m + 1]));
-        if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
-        if (m > 0) out.put(q[m + 1] + (Gp - G));     // eq. (38) for the cell between walk faces m-1 and m
-        Gp = G;
-        sig += ds;
+    for (int m0 = 0; m0 <= SEG; m0 += NB) {
+        double sp[NB], sm[NB];
+        bool need = false, needB = false;
+#pragma unroll
+        for (int i = 0; i < NB; ++i) {
+            const int m = m0 + i;
+            if (m > SEG) break;
+            const double f0 = q[m + 1];
+            sp[i] = q[m + 2] - f0; sm[i] = f0 - q[m];
+            if (LIM) {   // high-word test of slopes_fast: may a bound bind (conservative)?  Comparisons, not differences:
+                         // hf, hg are hugely negative for f0 < 0 or f0 > f_inf (round-off leaves -1e-17 behind)
+                const int hf = __double2hiint(f0) + 0x00100000, hg = __double2hiint(finf - f0) + 0x00100000;
+                const int hmax = max(__double2hiint(sp[i]) & 0x7fffffff, __double2hiint(sm[i]) & 0x7fffffff);
+                need |= hmax >= min(hf, hg);
+                needB |= hmax >= hg;
+            }
+        }
+        // (without FULL the lanes voting together are whoever is here right now: the votes only decide which of two
+        // equivalent evaluations runs, so any grouping that includes the lane itself is right)
+        if (LIM && __any_sync(FULL ? 0xffffffffu : __activemask(), need)) {
+            if (!__any_sync(FULL ? 0xffffffffu : __activemask(), needB)) {
+                // only the positivity bound 2 f0 can bind: eps+ d+ = min(d+, hiA), eps- d- = max(d-, -hiA)
+#pragma unroll
+                for (int i = 0; i < NB; ++i) {
+                    if (m0 + i > SEG) break;
+                    const double hiA = relu_bits(q[m0 + i + 1] + q[m0 + i + 1]), nA = -hiA;
+                    sp[i] = sp[i] < hiA ? sp[i] : hiA;
+                    sm[i] = sm[i] > nA ? sm[i] : nA;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < NB; ++i) {
+                    if (m0 + i > SEG) break;
+                    slopes_exact(q[m0 + i + 1], finf, sp[i], sm[i]);
+                }
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NB; ++i) {
+            const int m = m0 + i;
+            if (m > SEG) break;
+            const double bq = fabs(sig);
+            const double b2 = bq * bq;
+            const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
+            const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+            double G = bq * fma(c1, sp[i], fma(c2, sm[i], q[m + 1]));
+            if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
+            if (m > 0) out.put(q[m + 1] + (Gp - G));     // eq. (38) for the cell between walk faces m-1 and m
+            Gp = G;
+            sig += ds;
+        }
     }
 }
 
@@ -304,7 +359,7 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
 // s0 + s1 k (accumulated).  out.put(value) stores the new average of the next cell (a, a+1, ...).
 // FAST: 8-cell segments may take the flow-ordered walks (2: every lane of the warp is here).  LOOSE: the 4th cell
 // before a line is readable memory (any value), which admits floor|sigma| = 2 at a box face.
-template <int LIM, int FAST, int LOOSE = 0, class Out>
+template <int LIM, int FAST, int LOOSE = 0, int NB = 1, class Out>
 __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
                                             double finf, Out& out) {
     if (a >= b) return;                              // a trailing work item beyond the end of the line: nothing to do
@@ -318,7 +373,7 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
         constexpr int FULL = FAST == 2 ? 1 : 0;        // FAST == 2: every lane of the warp is here
         const unsigned mask = FULL ? 0xffffffffu : __activemask();
         if (__all_sync(mask, sub && !cross)) {
-            march_seg_small<SEG, LIM, FULL>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            march_seg_small<SEG, LIM, FULL, NB>(L, st8, N, a, sig, sig_b, s1, finf, out);
             return;
         }
         // march_seg_lite: its first face reads flow cells -3-n .. -1-n, with V_PAD zero cells before the line; the
@@ -464,7 +519,7 @@ __global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid
             const double s0 = t0 + t2 * k1 + t3 * k2;
             const int a = seg * seglen;
             OutGlobal o{fb + c + (long)a * plane, (long)plane};
-            march_cells<LIM, 2>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);     // whole warps take this together
+            march_cells<LIM, 2, 0, VL_X_BATCH>(smem_addr(A + c), CT * 8, N, a, a + seglen, s0, t1, finf, o);     // whole warps take this together
         }
         __syncthreads();                           // everybody is done reading buffer b: refill it
         if (threadIdx.x == 0 && tile + 2 * (int)gridDim.x < P.ntot) issue(tile + 2 * gridDim.x, b);
@@ -584,11 +639,17 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
 // no exposed load latency, two block barriers per tile instead of four, and still 3 CTAs per SM for 32x32 planes.
 //   shared: [staging: 8 + ct (CN + 8) rows of CN][Bf][A][mbarrier]
 // ------------------------------------------------------------------------------------------------
+// Tile shape of the TMA-staged vy+vz kernel for CN x CN planes: planes per tile (about 2048 cells), and the threads of
+// a CTA = one work item (an 8-cell segment of one line) per thread, rounded up to whole warps.
+__host__ __device__ constexpr int yz_tma_planes(int cn) { return 2048 / (cn * cn) > 0 ? 2048 / (cn * cn) : 1; }
+__host__ __device__ constexpr int yz_tma_threads(int cn) { return (yz_tma_planes(cn) * cn * ((cn + 7) / 8) + 31) / 32 * 32; }
+static_assert(yz_tma_threads(32) == 256 && yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(40) == 224, "");
+
 template <int LIM, int CN>
-__global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
+__global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
     extern __shared__ __align__(128) double sm[];
     constexpr int N1 = CN, N2 = CN, plane = CN * CN;
-    constexpr int ct = (8 * V_THREADS) / plane > 0 ? (8 * V_THREADS) / plane : 1;
+    constexpr int ct = yz_tma_planes(CN);
     constexpr int nseg = (CN + 7) / 8, seglen = (CN + nseg - 1) / nseg;
     constexpr int RS = N2 + V_PAD, PS = (N1 + V_PAD) * RS, OFF = V_PAD * RS + V_PAD;
     constexpr int BUF = (OFF + ct * PS + 1) & ~1;
@@ -596,7 +657,13 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
                                                                  // any even N2 keep every TMA box 128-byte aligned
     constexpr int SROWS = SPAD + ct * (N1 + SPAD);               // staging rows of N2 doubles
     constexpr int STG = (SROWS * N2 + 15) & ~15;                 // keeps Bf 128-byte aligned
-    constexpr int FW = (ct * CN * nseg) % V_THREADS == 0 ? 2 : 1; // 2: the work items fill whole warps (march_cells)
+    // The work items of a sweep (ct CN nseg) need not fill the last warp.  Its idle lanes REPEAT the items of the 32
+    // lanes before them (same reads, same values written to the same places), so that every warp that works at all is
+    // whole: the walks vote with the full mask, no __activemask() bookkeeping, no divergence guards around the votes.
+    constexpr int FW = 2;
+    constexpr int NITEM = ct * CN * nseg;
+    constexpr int NT = yz_tma_threads(CN);         // threads of the CTA: the work items rounded up to whole warps
+    static_assert(NITEM >= 32 && NITEM <= NT && NT - NITEM < 32 && CN % 8 == 0 && seglen == 8, "one item per thread, whole warps, whole segments");
     if (P.ct != ct || P.nseg != nseg || P.nseg2 != nseg || P.nv1 != CN || P.nv2 != CN) return;
     double* St = sm;
     double* Bf = sm + STG;
@@ -605,12 +672,12 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     const double* tab = A + BUF + 2;               // the tile's sweep-table row rides along with the tile (16-byte aligned)
     static_assert((TAB * 8) % 16 == 0, "bulk copy size");
     // zero: the staging pad rows (never written again), Bf and A entirely (their cells are overwritten per tile)
-    for (int e = threadIdx.x; e < SPAD * N2; e += V_THREADS) {
+    for (int e = threadIdx.x; e < SPAD * N2; e += NT) {
         St[e] = 0.0;
 #pragma unroll
         for (int p = 0; p < ct; ++p) St[(SPAD + p * (N1 + SPAD) + N1) * N2 + e] = 0.0;
     }
-    for (int e = threadIdx.x; e < 2 * BUF; e += V_THREADS) Bf[e] = 0.0;
+    for (int e = threadIdx.x; e < 2 * BUF; e += NT) Bf[e] = 0.0;
     if (threadIdx.x == 0) mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
@@ -630,7 +697,7 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
     const int z_init = threadIdx.x % N2, row_init = threadIdx.x / N2;
     const int y_init = row_init % N1;
     const unsigned so_init = OFF + (row_init / N1) * PS + y_init * RS + z_init;
-    constexpr int dz = V_THREADS % N2, drow = V_THREADS / N2, dy = drow % N1;
+    constexpr int dz = NT % N2, drow = NT / N2, dy = drow % N1;
     constexpr unsigned dso = dz + dy * RS + (drow / N1) * PS;
     constexpr int ncellt = ct * plane;
     int it = 0;
@@ -641,39 +708,50 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_tma_kernel(const __gri
         tcell += step_c; ttile += step_t;
         if (ttile >= P.ntile) { ttile -= P.ntile; ++tcell; }
         mbar_wait(bar, it & 1);
+        __syncwarp();                              // the store loop may end lane by lane: the warp is whole again here
         // the table row arrived with the tile; it is overwritten when the next tile is issued (after the vy sweep)
         const double ty0 = tab[4], ty1 = tab[5], ty2 = tab[6], ty3 = tab[7], finfy = tab[13];
         const double tz0 = tab[8], tz1 = tab[9], tz2 = tab[10], tz3 = tab[11], finfz = tab[14];
         {   // vy: line along i_vy (stride N2 in the staging buffer); transverse (plane, i_vz); threads run along z
             constexpr int nl = ct * N2;
-            for (int wi = threadIdx.x; wi < nl * nseg; wi += V_THREADS) {
+            {
+                int wi = threadIdx.x;
+                if (wi >= NITEM) wi -= 32;
                 const int seg = wi / nl, l = wi - seg * nl;
                 const int p = l / N2, z = l - p * N2;
                 const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
-                const int a = seg * seglen, b = min(a + seglen, N1);
+                const int a = seg * seglen, b = a + seglen;          // CN is a multiple of 8: whole segments
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM, FW, 1>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
+        __syncwarp();
         if (threadIdx.x == 0 && tile + (int)gridDim.x < P.ntot) issue(P.cell0 + tcell, ttile * ct);
         {   // vz: contiguous lines of Bf; transverse (plane, i_vy); threads run along y (pitch RS, odd)
             constexpr int nl = ct * N1;
-            for (int wi = threadIdx.x; wi < nl * nseg; wi += V_THREADS) {
+            {
+                int wi = threadIdx.x;
+                if (wi >= NITEM) wi -= 32;
                 const int seg = wi / nl, l = wi - seg * nl;
                 const int p = l / N1, y = l - p * N1;
                 const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
-                const int a = seg * seglen, b = min(a + seglen, N2);
+                const int a = seg * seglen, b = a + seglen;
                 OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
-                march_cells<LIM, FW, 1>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
             }
         }
         __syncthreads();                           // vz done: A complete
         {   // A -> global (the next tile's vz sweep writes A only after the next barrier)
+            // the same trip count for every lane (the last trip is guarded instead): a loop that ends lane by lane would
+            // make the compiler guard every full-mask vote of the next tile's walks against divergence
             int z = z_init, y = y_init;
             unsigned so = so_init;
-            for (int e = threadIdx.x; e < ncellt; e += V_THREADS) {
-                __stcs(fb + e, lds(sA + so * 8));
+            constexpr int NTRIP = (ncellt + NT - 1) / NT;
+#pragma unroll 2
+            for (int i = 0; i < NTRIP; ++i) {
+                const int e = threadIdx.x + i * NT;
+                if (ncellt % NT == 0 || e < ncellt) __stcs(fb + e, lds(sA + so * 8));
                 z += dz; y += dy; so += dso;
                 if (z >= N2) { z -= N2; so += RS - N2; ++y; }
                 if (y >= N1) { y -= N1; so += PS - N1 * RS; }
@@ -688,19 +766,19 @@ constexpr size_t V_SMEM_MAX = 200 * 1024;
 // Function attributes and occupancy are per device: the cache is keyed by (device, kernel, smem) and guarded, so
 // several contexts on several devices (or threads) of one process each get their own answer.
 template <class K>
-static int resident_ctas(K kernel, size_t smem) {
+static int resident_ctas(K kernel, size_t smem, int threads = V_THREADS) {
     static std::mutex mu;
     static std::map<std::tuple<int, const void*, size_t>, int> cache;
     int dev = 0;
     cudaGetDevice(&dev);
-    const auto key = std::make_tuple(dev, (const void*)kernel, smem);
+    const auto key = std::make_tuple(dev, (const void*)kernel, smem + ((size_t)threads << 40));
     std::lock_guard<std::mutex> lock(mu);
     auto it = cache.find(key);
     if (it != cache.end()) return it->second;
     cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V_SMEM_MAX);
     int per_sm = 0, sms = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, V_THREADS, smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem);
     if (per_sm < 1) per_sm = 1;
     cache[key] = per_sm * sms;
     return per_sm * sms;
@@ -790,9 +868,10 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
             const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8;
             if (smem_t > V_SMEM_MAX) return VLASOV_EINVAL;
-            const int grid = min(P.ntot, resident_ctas(kt, smem_t));
+            const int nt = spec == 16 ? yz_tma_threads(16) : spec == 24 ? yz_tma_threads(24) : spec == 40 ? yz_tma_threads(40) : yz_tma_threads(32);
+            const int grid = min(P.ntot, resident_ctas(kt, smem_t, nt));
             Launch L(c, K_VSWEEP_YZ);
-            kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);
+            kt<<<grid, nt, smem_t, c->stream>>>(tm, P);
         } else {
             const int grid = min(P.ntot, resident_ctas(k, smem));
             Launch L(c, K_VSWEEP_YZ);

@@ -60,6 +60,7 @@ struct vlasov_ctx {
     double* Bavg;        // [3][nyg*nx] B at the E time level of vlasov_cycle
     // optional per-kernel timing (vlasov_timing_*): event pairs around every launch
     int timing;
+    int ghost_tag;       // 1 while the launches being issued belong to the ghost fill / ghost rows (timing kinds)
     int nrec;
     static constexpr int MAX_REC = 8192;
     cudaEvent_t* ev0;    // [MAX_REC]
@@ -70,13 +71,21 @@ struct vlasov_ctx {
 namespace vl {
 
 enum Kind { K_SWEEP_X = 0, K_SWEEP_Y, K_TABLE, K_VSWEEP_X, K_VSWEEP_YZ, K_MOMENTS, K_GHOST_TABLE, K_CURRENT,
-            K_MAXWELL, K_SWEEP_XY, K_SWEEP_YX, K_COUNT };
+            K_MAXWELL, K_SWEEP_XY, K_SWEEP_YX, K_GHOST_VSWEEP_X, K_GHOST_VSWEEP_YZ, K_GHOST_MOMENTS, K_GHOST_SWEEP_X,
+            K_COUNT };
+static_assert((int)K_COUNT == (int)VLASOV_KIND_COUNT, "kinds of vlasov.h");
 
 // Counts a launch and, when timing is on, brackets it with an event pair on the context's stream.
 struct Launch {
     vlasov_ctx* c; int slot;
     Launch(vlasov_ctx* ctx, int kind) : c(ctx), slot(-1) {
         c->launches++;
+        if (c->ghost_tag) {      // work that only exists because a side is FLUID gets its own kind
+            if (kind == K_VSWEEP_X) kind = K_GHOST_VSWEEP_X;
+            else if (kind == K_VSWEEP_YZ) kind = K_GHOST_VSWEEP_YZ;
+            else if (kind == K_MOMENTS) kind = K_GHOST_MOMENTS;
+            else if (kind == K_SWEEP_X) kind = K_GHOST_SWEEP_X;
+        }
         if (c->timing && c->nrec < vlasov_ctx::MAX_REC) {
             slot = c->nrec++;
             c->rec_kind[slot] = kind;
@@ -201,6 +210,23 @@ __device__ __forceinline__ void slopes_fast(double fm, double f0, double fp, dou
             }
         }
     }
+}
+
+// The exact clamps of slopes_fast (both bounds), applied in place to the raw differences sp = d+, sm = d- of a cell
+// with value f0: |eps d| = min(|d|, bound picked by the sign of d), sign restored.
+__device__ __forceinline__ void slopes_exact(double f0, double finf, double& sp, double& sm) {
+    const double dp = sp, dm = sm, g = finf - f0;
+    const double hiA = relu_bits(f0 + f0), hiB = relu_bits(g + g);
+    const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
+    const bool pneg = __double2hiint(dp) < 0, mneg = __double2hiint(dm) < 0;
+    const double bp = pneg ? hiB : hiA;
+    const double bm = mneg ? hiA : hiB;
+    const double ap = __hiloint2double(hp, __double2loint(dp));      // |d+|
+    const double am = __hiloint2double(hm, __double2loint(dm));      // |d-|
+    const double mp = ap < bp ? ap : bp;
+    const double mm = am < bm ? am : bm;
+    sp = __hiloint2double(__double2hiint(mp) | (__double2hiint(dp) & 0x80000000), __double2loint(mp));
+    sm = __hiloint2double(__double2hiint(mm) | (__double2hiint(dm) & 0x80000000), __double2loint(mm));
 }
 
 // n = floor(s) for s >= 0 up to the exact-integer case, where n = s - 1, b = 1 is returned instead:
