@@ -242,7 +242,8 @@ def gpu_arm(args):
     fs = [upload_f(w, s, torch, device) for s in range(ns)]
     E0, B0 = inputs.gem_fields(w)
     stream = torch.cuda.current_stream()
-    ctx = binding.context_for(w, fs)
+    order = binding.ORDER_VXV if args.order == "vxv" else binding.ORDER_XVX
+    ctx = binding.context_for(w, fs, order=order)
     Ed, Bd = torch.from_numpy(E0).to(device), torch.from_numpy(B0).to(device)
     fluid = None
     if w.bc_y_lo == inputs.BC_FLUID:
@@ -412,7 +413,8 @@ def gpu_arm(args):
         "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise, DESIGN.md 'Input recipe')",
         "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nghost_y": w.nghost_y,
                    "nv": list(w.species[0].nv), "species": ns, "dt": w.dt, "maxwell_nsub": w.nsub,
-                   "interior_cells_per_step": cells, "order": "XVX (eq. 22)", "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "interior_cells_per_step": cells,
+                   "order": "VXV (PAPER.md:420; moments fused into the last vy+vz pass)" if args.order == "vxv" else "XVX (eq. 22)", "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: {sum(f.numel() for f in fs) * 8 / 1e9:.2f} GB of f streamed by every pass (L2 126 MB)"},
         "clocks": clocks,
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
@@ -465,6 +467,7 @@ def main():
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed block of --steps cycles (median reported)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="gem128")
+    ap.add_argument("--order", default="xvx", choices=["xvx", "vxv"], help="Strang order of the Vlasov step (R2); xvx is the benchmark")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle time for the cpu_baseline leg")
     ap.add_argument("--ref-budget", type=float, default=150.0, help="seconds of oracle time for --impl reference")

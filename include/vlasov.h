@@ -175,8 +175,11 @@ int vlasov_timing_read(vlasov_ctx* ctx, double* ms_by_kind, int64_t* count_by_ki
 
 /* Execution options (results stay within the parity tolerance either way).
  * VLASOV_OPT_FUSE_XY (default 1): run each spatial stage (x/2 y/2, y/2 x/2) as ONE fused pass over f when every
- * shift of the stage is below one cell; 0 = always the general one-direction kernels.  Errors: EINVAL. */
-enum { VLASOV_OPT_FUSE_XY = 1 };
+ * shift of the stage is below one cell; 0 = always the general one-direction kernels.  Errors: EINVAL.
+ * VLASOV_OPT_FUSE_MOMENTS (default 1): ORDER_VXV only: reduce the moments of the final f inside the last
+ * velocity pass (vy+vz kernel, 16^3 / 32^3 velocity blocks) instead of a separate pass over f; 0 = always the separate
+ * moments kernel. */
+enum { VLASOV_OPT_FUSE_XY = 1, VLASOV_OPT_FUSE_MOMENTS = 2 };
 int vlasov_set_option(vlasov_ctx* ctx, int option, int value);
 
 /* Tell the library the caller wrote into an f buffer itself (drops the kept moments). */

@@ -21,6 +21,7 @@ EXPORTS = ["vlasov_scratch_bytes", "vlasov_init", "vlasov_set_boundary", "vlasov
            "vlasov_launch_count", "vlasov_free", "vlasov_strerror", "vlasov_cycle", "vlasov_cycle_host",
            "vlasov_timing_enable", "vlasov_timing_read", "vlasov_fluid_boundary_mark", "vlasov_fluid_boundary"]
 OPT_FUSE_XY = 1
+OPT_FUSE_MOMENTS = 2
 KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy", "sweep_yx",
          "ghost_vsweep_x", "ghost_vsweep_yz", "ghost_moments", "ghost_sweep_x"]
 

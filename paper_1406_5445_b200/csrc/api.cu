@@ -78,24 +78,35 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         r = launch_sweep_y(c, s, cur, other, dts); if (r) return r;
         return launch_sweep_x(c, s, other, cur, dts);
     };
-    auto velocity = [&](double dtv) -> int {
+    bool mom_done = false;
+    // flips_after: how many fused (one pass, buffer-swapping) spatial stages still follow in this call.  The vx sweep
+    // can read one buffer and write the other, so the velocity step is where f changes sides for free: it leaves f
+    // where the remaining stages bring it home to the caller's buffer without a copy.
+    auto velocity = [&](double dtv, int flips_after, bool with_moments = false) -> int {
         int r = launch_lorentz_table(c, s, E, B, dtv); if (r) return r;
-        return launch_vsweeps(c, s, cur, 0, G.nyg);      // ghost rows too (R16)
+        double* target = (flips_after & 1) ? c->pong : s.f;
+        // with_moments (the last pass of a VXV step): the moments of the final f may be reduced by the vy+vz kernel
+        // itself.  All rows, ghost rows too (R16).
+        double* mo = with_moments && c->fuse_mom && target == s.f ? c->mom + (long)si * 11 * ((long)G.nyg * G.nx) : nullptr;
+        r = launch_vsweeps(c, s, target, 0, G.nyg, false, mo, &mom_done, cur);
+        cur = target;
+        return r;
     };
+    auto flips = [&](bool requested, double dts) { return requested && c->fuse_xy && fused_xy_applicable(c, s, dts) ? 1 : 0; };
     if (c->order == VLASOV_ORDER_XVX) {
         if (stages & VLASOV_STAGE_X1) { e = space(dt / 2.0, true); if (e) return e; }
-        if (stages & VLASOV_STAGE_V) { e = velocity(dt); if (e) return e; }
+        if (stages & VLASOV_STAGE_V) { e = velocity(dt, flips((stages & VLASOV_STAGE_X2) != 0, dt / 2.0)); if (e) return e; }
         if (stages & VLASOV_STAGE_X2) { e = space(dt / 2.0, false); if (e) return e; }     // palindrome, R3
     } else {
-        if (stages & VLASOV_STAGE_X1) { e = velocity(dt / 2.0); if (e) return e; }
+        if (stages & VLASOV_STAGE_X1) { e = velocity(dt / 2.0, flips((stages & VLASOV_STAGE_V) != 0, dt)); if (e) return e; }
         if (stages & VLASOV_STAGE_V) { e = space(dt, true); if (e) return e; }
-        if (stages & VLASOV_STAGE_X2) { e = velocity(dt / 2.0); if (e) return e; }
+        if (stages & VLASOV_STAGE_X2) { e = velocity(dt / 2.0, 0, (stages & VLASOV_STAGE_MOMENTS) != 0); if (e) return e; }
     }
     if (cur != s.f) {
         VL_CUDA_OK(cudaMemcpyAsync(s.f, cur, (size_t)G.nyg * G.nx * s.nvtot * 8, cudaMemcpyDeviceToDevice, c->stream));
         c->launches++;
     }
-    if (stages & VLASOV_STAGE_MOMENTS) {
+    if ((stages & VLASOV_STAGE_MOMENTS) && !mom_done) {
         const long ncell = (long)G.nyg * G.nx;
         e = launch_moments(c, s, s.f, c->mom + (long)si * 11 * ncell, 0, G.nyg); if (e) return e;
     }
@@ -186,6 +197,7 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     c->timing = 0; c->ghost_tag = 0; c->nrec = 0; c->ev0 = c->ev1 = nullptr; c->rec_kind = nullptr;
     c->mom_valid = 0;
     c->fuse_xy = 1;
+    c->fuse_mom = 1;
     c->launches = 0;
     c->h_err = nullptr;
     if (cudaMallocHost((void**)&c->h_err, sizeof(int)) != cudaSuccess) { delete c; return VLASOV_ECUDA; }
@@ -359,6 +371,7 @@ int vlasov_maxwell(vlasov_ctx* c, double dt, int nsub, double* E_dev, double* B_
 int vlasov_set_option(vlasov_ctx* c, int option, int value) {
     if (!c) return VLASOV_EINVAL;
     if (option == VLASOV_OPT_FUSE_XY) { c->fuse_xy = value ? 1 : 0; return VLASOV_OK; }
+    if (option == VLASOV_OPT_FUSE_MOMENTS) { c->fuse_mom = value ? 1 : 0; return VLASOV_OK; }
     return VLASOV_EINVAL;
 }
 

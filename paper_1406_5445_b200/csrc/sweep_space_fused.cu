@@ -52,13 +52,12 @@ struct Weights {
 };
 
 // Does the slope pair (dp, dm) of a cell with value f0 possibly need limiting?  High-word test of
-// vlasov_internal.cuh (conservative).  Returns a word whose sign bit is set if so.
-__device__ __forceinline__ int need_bits(double f0, double dp, double dm, double finf) {
-    // f0 < 0 or f0 > f_inf (round-off leaves -1e-17 behind): the high word is hugely negative, and the difference
-    // below would wrap around; max(., 0) keeps the answer "yes" there
-    const int hb = max(min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000, 0);
+// vlasov_internal.cuh (conservative).  A comparison, not a difference: for f0 < 0 or f0 > f_inf (round-off leaves
+// -1e-17 behind) the high word of the bound is hugely negative and a difference would wrap around.
+__device__ __forceinline__ bool may_need(double f0, double dp, double dm, double finf) {
+    const int hb = min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000;
     const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
-    return (hb - 1) - max(hp, hm);
+    return max(hp, hm) >= hb;
 }
 
 // N partial fluxes alpha [ f0 + c1 eps+ d+ + c2 eps- d- ] of the cells q[1..N] of a line piece q[0..N+1]
@@ -70,10 +69,10 @@ __device__ __forceinline__ void flux_line(const double (&q)[N + 2], const Weight
 #pragma unroll
     for (int i = 0; i <= N; ++i) d[i] = q[i + 1] - q[i];
     if (LIM) {
-        int need = 0;
+        bool need = false;
 #pragma unroll
-        for (int i = 0; i < N; ++i) need |= need_bits(q[i + 1], d[i + 1], d[i], finf);
-        if (__any_sync(__activemask(), need < 0)) {
+        for (int i = 0; i < N; ++i) need |= may_need(q[i + 1], d[i + 1], d[i], finf);
+        if (__any_sync(__activemask(), need)) {
 #pragma unroll
             for (int i = 0; i < N; ++i) {
                 double sp, sm;
@@ -117,13 +116,13 @@ template <int NB, int LIM>
 __device__ __forceinline__ void y_batch(const double (&ya)[NB], const double (&yb)[NB], double (&yG)[NB],
                                         const double (&gx)[NB], const Weights& Wy, double finf, double (&h)[NB]) {
     double dlo[NB], dhi[NB];
-    int need = 0;
+    bool need = false;
 #pragma unroll
     for (int i = 0; i < NB; ++i) {
         dlo[i] = yb[i] - ya[i]; dhi[i] = gx[i] - yb[i];
-        if (LIM) need |= need_bits(yb[i], dhi[i], dlo[i], finf);
+        if (LIM) need |= may_need(yb[i], dhi[i], dlo[i], finf);
     }
-    const bool slow = LIM && __any_sync(__activemask(), need < 0);
+    const bool slow = LIM && __any_sync(__activemask(), need);
 #pragma unroll
     for (int i = 0; i < NB; ++i) {
         double sp = Wy.pos ? dhi[i] : -dlo[i], sm = Wy.pos ? dlo[i] : -dhi[i];

@@ -191,16 +191,6 @@ struct OutGlobal {       // cells of a line in global memory (streaming store)
     __device__ __forceinline__ void skip(int n) { p += n * st; }
 };
 
-// Does the slope pair (dp, dm) of a cell with value f0 possibly need limiting?  High-word test of slopes_fast
-// (conservative).  The sign bit of the result is set if so.
-__device__ __forceinline__ int need_bits(double f0, double dp, double dm, double finf) {
-    // f0 < 0 or f0 > f_inf (round-off leaves -1e-17 behind): the high word is hugely negative, and the difference
-    // below would wrap around; max(., 0) keeps the answer "yes" there
-    const int hb = max(min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000, 0);
-    const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
-    return (hb - 1) - max(hp, hm);
-}
-
 // Segment of SEG cells [a, a+SEG) whose SEG+1 faces all have |sigma| < 1 (no whole cells in eqs. 46/47) and one
 // flow direction: the SEG+3 cells the fluxes touch are read ONCE into registers, in the direction of the flow
 // (eq. 47 = eq. 46 on the mirrored line), and face m of the walk takes (q[m], q[m+1], q[m+2]).  About a
@@ -224,6 +214,23 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
     if (!pos) { out.skip(SEG - 1); }
     out.step(dir);
     double Gp = 0.0;
+    if constexpr (NB == 1) {
+        // one limiter vote per face (slopes_fast): the leanest form in registers, for the kernel that has none to spare
+#pragma unroll
+        for (int m = 0; m <= SEG; ++m) {
+            double sp, sm;
+            slopes_fast<LIM, FULL>(q[m], q[m + 1], q[m + 2], finf, sp, sm);
+            const double bq = fabs(sig);
+            const double b2 = bq * bq;
+            const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
+            const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+            double G = bq * fma(c1, sp, fma(c2, sm, q[m + 1]));
+            if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
+            if (m > 0) out.put(q[m + 1] + (Gp - G));     // eq. (38) for the cell between walk faces m-1 and m
+            Gp = G;
+            sig += ds;
+        }
+    } else
     // NB faces at a time: ONE limiter vote per batch (all lanes sit on the same faces), so that the NB flux
     // evaluations are independent instruction streams between the votes
 #pragma unroll
@@ -404,6 +411,7 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
 }
 
 struct VParams {
+    const double* fsrc;   // what the vx sweep READS (== f: in place; the ping-pong buffer after a fused spatial stage)
     double* __restrict__ f;
     const double* __restrict__ table;
     long S;
@@ -414,6 +422,10 @@ struct VParams {
     int ntot;         // tiles of this launch
     int nseg;         // threads per line (vx kernel; vy lines of the vyz kernel)
     int nseg2;        // threads per vz line
+    // moments fused into the vy+vz kernel (VXV order, NEXT-1): out[10][mom_ncell] of the cells of this launch, or null
+    double* __restrict__ mom;
+    int mom_ncell;
+    double vmin[3], dv[3];
 };
 
 constexpr int V_THREADS = 256;
@@ -441,7 +453,7 @@ __global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams
         const int ncol = min(CT, plane - c0);
         const double* T = P.table + (long)cell * TAB;
         const double t0 = T[0], t1 = T[1], t2 = T[2], t3 = T[3], finf = T[12], scale = T[15];
-        const double* fsrc = P.f + (long)T[16] * P.S + c0;
+        const double* fsrc = P.fsrc + (long)T[16] * P.S + c0;
         double* fb = P.f + (long)cell * P.S + c0;
         for (int e = threadIdx.x; e < N * H; e += V_THREADS) {
             const int k = e / H, c = 2 * (e - k * H);
@@ -645,7 +657,11 @@ __host__ __device__ constexpr int yz_tma_planes(int cn) { return 2048 / (cn * cn
 __host__ __device__ constexpr int yz_tma_threads(int cn) { return (yz_tma_planes(cn) * cn * ((cn + 7) / 8) + 31) / 32 * 32; }
 static_assert(yz_tma_threads(32) == 256 && yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(40) == 224, "");
 
-template <int LIM, int CN>
+// MOM = 1 (VXV order): the 10 raw velocity moments, eqs. (2)-(4), of the final f are
+// reduced in this kernel.  A CTA then takes WHOLE spatial cells (all tiles of a cell one after the other), sums its
+// cells while it stores them, and writes the moments of the cell itself: no partial sums in global memory, no
+// atomics, a fixed summation order.  For planes where a thread keeps its i_vz over a tile (16x16, 32x32).
+template <int LIM, int CN, int MOM = 0>
 __global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
     extern __shared__ __align__(128) double sm[];
     constexpr int N1 = CN, N2 = CN, plane = CN * CN;
@@ -670,6 +686,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_
     double* A = Bf + BUF;
     const unsigned bar = smem_addr(A + BUF);
     const double* tab = A + BUF + 2;               // the tile's sweep-table row rides along with the tile (16-byte aligned)
+    double* red = A + BUF + 2 + TAB;               // MOM: [warps][10] partial sums of a spatial cell
     static_assert((TAB * 8) % 16 == 0, "bulk copy size");
     // zero: the staging pad rows (never written again), Bf and A entirely (their cells are overwritten per tile)
     for (int e = threadIdx.x; e < SPAD * N2; e += NT) {
@@ -689,10 +706,13 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_
         for (int p = 0; p < ct; ++p)
             tma_g2s_2d(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2) * 8, &tmap, 0, (cell * P.nv0 + p0 + p) * N1, bar);
     };
-    // (spatial cell, tile within the cell) of this CTA's tiles, advanced without a division per tile
-    const int step_c = gridDim.x / P.ntile, step_t = gridDim.x % P.ntile;
-    int tcell = blockIdx.x / P.ntile, ttile = blockIdx.x % P.ntile;
-    if (threadIdx.x == 0 && (int)blockIdx.x < P.ntot) issue(P.cell0 + tcell, ttile * ct);
+    // (spatial cell, tile within the cell) of this CTA's tiles, advanced without a division per tile.  MOM: the CTA
+    // owns the cells blockIdx.x, blockIdx.x + gridDim.x, ... and walks the tiles of a cell in order.
+    const int step_c = MOM ? 0 : gridDim.x / P.ntile, step_t = MOM ? 1 : gridDim.x % P.ntile;
+    const int wrap_c = MOM ? gridDim.x : 1;
+    const int ncell_l = P.ntot / P.ntile;
+    int tcell = MOM ? blockIdx.x : blockIdx.x / P.ntile, ttile = MOM ? 0 : blockIdx.x % P.ntile;
+    if (threadIdx.x == 0 && tcell < ncell_l) issue(P.cell0 + tcell, ttile * ct);
     // staging map of the store loop (as in the plain kernel)
     const int z_init = threadIdx.x % N2, row_init = threadIdx.x / N2;
     const int y_init = row_init % N1;
@@ -700,15 +720,17 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_
     constexpr int dz = NT % N2, drow = NT / N2, dy = drow % N1;
     constexpr unsigned dso = dz + dy * RS + (drow / N1) * PS;
     constexpr int ncellt = ct * plane;
+    double T0 = 0.0, Tx = 0.0, Txx = 0.0, Ty = 0.0, Tyy = 0.0, Txy = 0.0;      // MOM: this thread's sums over a spatial cell
     int it = 0;
-    for (int tile = blockIdx.x; tile < P.ntot; tile += gridDim.x, ++it) {
+    for (; tcell < ncell_l; ++it) {
         const int cell = P.cell0 + tcell;
         const int p0 = ttile * ct;
         double* fb = P.f + (long)cell * P.S + (long)p0 * plane;
         tcell += step_c; ttile += step_t;
-        if (ttile >= P.ntile) { ttile -= P.ntile; ++tcell; }
+        const bool last_of_cell = ttile >= P.ntile;
+        if (last_of_cell) { ttile -= P.ntile; tcell += wrap_c; }
         mbar_wait(bar, it & 1);
-        __syncwarp();                              // the store loop may end lane by lane: the warp is whole again here
+        if (NT != V_THREADS) __syncwarp();
         // the table row arrived with the tile; it is overwritten when the next tile is issued (after the vy sweep)
         const double ty0 = tab[4], ty1 = tab[5], ty2 = tab[6], ty3 = tab[7], finfy = tab[13];
         const double tz0 = tab[8], tz1 = tab[9], tz2 = tab[10], tz3 = tab[11], finfz = tab[14];
@@ -726,8 +748,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
-        __syncwarp();
-        if (threadIdx.x == 0 && tile + (int)gridDim.x < P.ntot) issue(P.cell0 + tcell, ttile * ct);
+        if (threadIdx.x == 0 && tcell < ncell_l) issue(P.cell0 + tcell, ttile * ct);
         {   // vz: contiguous lines of Bf; transverse (plane, i_vy); threads run along y (pitch RS, odd)
             constexpr int nl = ct * N1;
             {
@@ -742,19 +763,71 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_
             }
         }
         __syncthreads();                           // vz done: A complete
+        if (MOM) {
+            // A -> global, and the sums of the stored cells.  This thread keeps its i_vz; per plane its cells are EPP rows
+            // drow apart: sum f, sum vy f, sum vy^2 f over them, folded with the plane's vx; vz enters once per spatial cell.
+            static_assert(!MOM || (dz == 0 && N1 % drow == 0 && ncellt % NT == 0), "fused moments: a thread keeps its i_vz");
+            constexpr int EPP = N1 / (drow > 0 ? drow : 1);
+            const double vy0 = P.vmin[1] + (y_init + 0.5) * P.dv[1];
+#pragma unroll
+            for (int pp = 0; pp < ct; ++pp) {
+                double r0 = 0.0, r1 = 0.0, r2 = 0.0;
+#pragma unroll
+                for (int j = 0; j < EPP; ++j) {
+                    const double fv = lds(sA + (so_init + pp * PS + j * drow * RS) * 8);
+                    __stcs(fb + threadIdx.x + (pp * EPP + j) * NT, fv);
+                    const double vy = vy0 + (j * drow) * P.dv[1];
+                    const double t = vy * fv;
+                    r0 += fv; r1 += t; r2 = fma(vy, t, r2);
+                }
+                const double vx = P.vmin[0] + (p0 + pp + 0.5) * P.dv[0];
+                const double u = vx * r0;
+                T0 += r0; Tx += u; Txx = fma(vx, u, Txx); Ty += r1; Tyy += r2; Txy = fma(vx, r1, Txy);
+            }
+            if (last_of_cell) {
+                const double vz = P.vmin[2] + (z_init + 0.5) * P.dv[2];
+                double M[10] = {T0, Tx, Ty, vz * T0, Txx, Tyy, vz * (vz * T0), Txy, vz * Tx, vz * Ty};
+                T0 = Tx = Txx = Ty = Tyy = Txy = 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int q = 0; q < 10; ++q) M[q] += __shfl_down_sync(0xffffffffu, M[q], o);
+                }
+                if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+                    for (int q = 0; q < 10; ++q) red[(threadIdx.x >> 5) * 10 + q] = M[q];
+                }
+                __syncthreads();
+                if (threadIdx.x < 10) {
+                    double r = red[threadIdx.x];
+                    for (int w = 1; w < NT / 32; ++w) r += red[w * 10 + threadIdx.x];      // fixed order over the warps
+                    P.mom[(long)threadIdx.x * P.mom_ncell + (cell - P.cell0)] = r * (P.dv[0] * P.dv[1] * P.dv[2]);
+                }
+                // red is written again a whole spatial cell (>= 2 block barriers) later
+            }
+        } else
         {   // A -> global (the next tile's vz sweep writes A only after the next barrier)
             // the same trip count for every lane (the last trip is guarded instead): a loop that ends lane by lane would
             // make the compiler guard every full-mask vote of the next tile's walks against divergence
             int z = z_init, y = y_init;
             unsigned so = so_init;
             constexpr int NTRIP = (ncellt + NT - 1) / NT;
-#pragma unroll 2
-            for (int i = 0; i < NTRIP; ++i) {
-                const int e = threadIdx.x + i * NT;
-                if (ncellt % NT == 0 || e < ncellt) __stcs(fb + e, lds(sA + so * 8));
-                z += dz; y += dy; so += dso;
-                if (z >= N2) { z -= N2; so += RS - N2; ++y; }
-                if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+            if constexpr (ncellt % NT == 0) {
+                for (int e = threadIdx.x; e < ncellt; e += NT) {
+                    __stcs(fb + e, lds(sA + so * 8));
+                    z += dz; y += dy; so += dso;
+                    if (z >= N2) { z -= N2; so += RS - N2; ++y; }
+                    if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+                }
+            } else {
+#pragma unroll 4
+                for (int i = 0; i < NTRIP; ++i) {
+                    const int e = threadIdx.x + i * NT;
+                    if (e < ncellt) __stcs(fb + e, lds(sA + so * 8));
+                    z += dz; y += dy; so += dso;
+                    if (z >= N2) { z -= N2; so += RS - N2; ++y; }
+                    if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+                }
             }
         }
     }
@@ -784,12 +857,17 @@ static int resident_ctas(K kernel, size_t smem, int threads = V_THREADS) {
     return per_sm * sms;
 }
 
-int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost) {
+int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost, double* mom_out, bool* mom_done,
+                   const double* src) {
+    if (!src) src = f;
+    if (mom_done) *mom_done = false;
     if (nrows <= 0) return VLASOV_OK;
     VParams P;
-    P.f = f; P.table = c->table; P.S = s.nvtot;
+    P.fsrc = src; P.f = f; P.table = c->table; P.S = s.nvtot;
     P.nv0 = s.nv[0]; P.nv1 = s.nv[1]; P.nv2 = s.nv[2];
     P.cell0 = row0 * c->G.nx;
+    P.mom = nullptr; P.mom_ncell = 0;
+    for (int d = 0; d < 3; ++d) { P.vmin[d] = s.vmin[d]; P.dv[d] = s.dv[d]; }
     const int lim = c->G.limiter ? 1 : 0;
     const int ncell = nrows * c->G.nx;
     const int plane = s.nv[1] * s.nv[2];
@@ -813,7 +891,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (tspec && !ghost && (long)c->G.nyg * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
             // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]; its own tile shape
             CUtensorMap tm;
-            if (!make_tensor_map_2d(&tm, f, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, tspec)) return VLASOV_ECUDA;
+            if (!make_tensor_map_2d(&tm, src, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, tspec)) return VLASOV_ECUDA;
             P.ct = 128; P.nseg = tspec / 8;
             P.ntile = (plane + 127) / 128;
             P.ntot = P.ntile * ncell;
@@ -866,10 +944,18 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (spec == 40) kt = lim ? vsweep_yz_tma_kernel<1, 40> : vsweep_yz_tma_kernel<0, 40>;
             const size_t srows = 8 + (size_t)pt * (s.nv[1] + 8);
             const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
-            const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8;
+            const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8 + 8 * 10 * 8;
+            // moments of the final f reduced in the same pass (VXV order): CTAs take whole spatial cells
+            const bool mom = mom_out && !ghost && (spec == 16 || spec == 32);
+            if (mom) {
+                P.mom = mom_out; P.mom_ncell = ncell;
+                if (spec == 16) kt = lim ? vsweep_yz_tma_kernel<1, 16, 1> : vsweep_yz_tma_kernel<0, 16, 1>;
+                else kt = lim ? vsweep_yz_tma_kernel<1, 32, 1> : vsweep_yz_tma_kernel<0, 32, 1>;
+                if (mom_done) *mom_done = true;
+            }
             if (smem_t > V_SMEM_MAX) return VLASOV_EINVAL;
             const int nt = spec == 16 ? yz_tma_threads(16) : spec == 24 ? yz_tma_threads(24) : spec == 40 ? yz_tma_threads(40) : yz_tma_threads(32);
-            const int grid = min(P.ntot, resident_ctas(kt, smem_t, nt));
+            const int grid = min(mom ? ncell : P.ntot, resident_ctas(kt, smem_t, nt));
             Launch L(c, K_VSWEEP_YZ);
             kt<<<grid, nt, smem_t, c->stream>>>(tm, P);
         } else {

@@ -54,6 +54,7 @@ struct vlasov_ctx {
     int* errflag;        // device int: first asynchronous error
     int mom_valid;
     int fuse_xy;         // 1: use the fused spatial stage where it applies (vlasov_set_option)
+    int fuse_mom;        // 1: VXV order: reduce the moments in the last vy+vz pass where that kernel can
     int64_t launches;
     int* h_err;          // pinned host mirror of errflag
     double* Jbuf;        // [3][nyg*nx] current density of vlasov_cycle
@@ -109,7 +110,10 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
 // Lorentz table (a3) and velocity sweeps (a4-a6), in place on f, rows [row0, row0+nrows)
 int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const double* B, double dt);
 // ghost: the launch is a ghost fill (tiles read the edge cell T[16] and are scaled by T[15])
-int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost = false);
+// mom_out: if not null, [11][nrows*nx] moments of the swept rows MAY be reduced in the same pass (*mom_done tells).
+// src: if not null, the vx sweep reads src and writes f (out of place; vy and vz then run in place on f).
+int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nrows, bool ghost = false,
+                   double* mom_out = nullptr, bool* mom_done = nullptr, const double* src = nullptr);
 // moments (a9): out[11][nyg*nx] (10 moments + max f) of rows [row0,row0+nrows) of f
 int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out, int row0, int nrows);
 // ghost fill (a0) of one side

@@ -716,3 +716,42 @@ def test_init_and_step_refusals(gpu):
     ctx.vlasov_step(0.01, Z, Z, gpu.STAGE_ALL & ~gpu.STAGE_GHOST)      # without the ghost stage the caller's rows are used
     assert ctx.check_code() == 0
     ctx.close()
+
+
+@pytest.mark.parametrize("nv", [(32, 32, 32), (16, 16, 16), (24, 24, 24)])
+def test_vxv_step_with_moments_fused_into_the_last_velocity_pass(gpu, orc, nv):
+    """NEXT-1: the order of the paper's coupled cycle, v/2 - x,y - v/2, with the 10 moments
+    of the final f reduced inside the last vy+vz pass (16^3 and 32^3 blocks: no separate moments launch; 24^3 keeps
+    the moments kernel).  f and moments against the oracle's VXV step (pinned by T10/T12/T16 under order = 1), and
+    against the same step with the fusion switched off."""
+    import torch
+    rng = np.random.default_rng(17)
+    w = random_workload(rng, nx=5, ny=3, nv=nv, bc=inputs.BC_REFLECT, nspecies=2, fields_yee=1, vmax=(4.0, 3.0, 3.5))
+    f0 = [smooth_random_f(rng, w, s) for s in range(2)]
+    E = rng.standard_normal((3, w.ny_g, w.nx))
+    B = 1.5 * rng.standard_normal((3, w.ny_g, w.nx))
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, 0.05, 31, order=1)
+    assert code == 0
+    k = run_both.kinds
+    fused = nv[0] in (16, 32)
+    assert k["vsweep_yz"][1] == 4 and k["moments"][1] == (0 if fused else 2), k
+    for s in range(2):
+        assert rel_l2(fg[s], fo[s]) <= TOL1
+        assert np.abs(fg[s] - fo[s]).max() <= 2e-13
+        assert rel_l2(mg[s], mo[s]) <= TOL1
+        for q in range(10):                       # every moment on its own (the small ones too)
+            assert np.abs(mg[s][q] - mo[s][q]).max() <= 1e-12 * np.abs(mo[s][[0, 4, 5, 6]]).max(), (s, q)
+    # the same step with the separate moments kernel
+    fg2 = [dev(f) for f in f0]
+    ctx = gpu.context_for(w, fg2, order=1)
+    ctx.vlasov_set_option(gpu.OPT_FUSE_MOMENTS, 0)
+    ctx.vlasov_timing_enable(True)
+    ctx.vlasov_step(0.05, dev(E), dev(B), 31)
+    assert ctx.check_code() == 0
+    assert ctx.vlasov_timing_read()["moments"][1] == 2
+    m = torch.empty((10, w.ny_g, w.nx), dtype=torch.float64, device="cuda")
+    for s in range(2):
+        ctx.vlasov_moments(s, m)
+        assert np.array_equal(fg2[s].cpu().numpy(), fg[s])
+        assert rel_l2(m.cpu().numpy(), mg[s]) <= 1e-14
+    ctx.close()
