@@ -194,6 +194,37 @@ int64_t vlasov_launch_count(const vlasov_ctx* ctx);
 void vlasov_free(vlasov_ctx* ctx);
 const char* vlasov_strerror(int err);
 
+/* ---- the fluid side of the coupling (section 3.2; cycle item 4 PAPER.md:421) ----------
+ * Five-moment fluid step per species: the moment equations (5)-(7) PAPER.md:50-54 with the adiabatic closure (8)
+ * PAPER.md:61 and the Lorentz source, "CWENO scheme [18] ... third order strong-stability-preserving Runge-Kutta scheme
+ * by Shu and Osher [19]" (details: reading R23 of DESIGN.md).  Stateless: no context, every array is the caller's.
+ *   U_dev      [nspecies][5][ny + 4][nx]  cell averages of rho, u_x, u_y, u_z (MOMENTUM density, eq. 3), energy density;
+ *              two ghost rows per y side (scratch unless the side is COUPLED ... and then they are overwritten too)
+ *   E_dev, B_dev  [3][ny + 4][nx]  fields at the cell centres, held fixed over the step
+ *   ghost_lo_dev, ghost_hi_dev  [3][nspecies][5][2][nx]  ghost rows (ascending y) of a COUPLED side at the three
+ *              Runge-Kutta stage times t, t + dt, t + dt/2 -- in this order (section 4.1: "needs boundary
+ *              conditions at times t, t + dt/2 and t + dt ... by linear interpolation in time"); NULL for other kinds
+ * x is periodic.  Errors: EINVAL, EALIGN, ECUDA. */
+enum { VLASOV_FLUID_BC_PERIODIC = 0, VLASOV_FLUID_BC_WALL = 1 /* mirror image, u_y odd */, VLASOV_FLUID_BC_COUPLED = 2 };
+enum { VLASOV_FLUID_MAX_SPECIES = 8 };
+typedef struct {
+    int32_t nx, ny;          /* interior cells of the fluid block */
+    int32_t nspecies;
+    int32_t bc_y_lo, bc_y_hi;
+    int32_t reserved;
+    double dx, dy;
+    double q[VLASOV_FLUID_MAX_SPECIES], m[VLASOV_FLUID_MAX_SPECIES];
+    void* stream;            /* cudaStream_t */
+} vlasov_fluid_config;
+size_t vlasov_fluid_scratch_bytes(const vlasov_fluid_config* cfg);
+int vlasov_fluid_step(const vlasov_fluid_config* cfg, double dt, double* U_dev, const double* E_dev, const double* B_dev,
+                      const double* ghost_lo_dev, const double* ghost_hi_dev, void* scratch_dev, size_t scratch_bytes);
+/* eqs. (2)-(4) PAPER.md:39-46: rho = m M0, u = m M1, energy = (m/2)(M2xx + M2yy + M2zz) from raw moments [10][n] (the
+ * layout of vlasov_moments / vlasov_fluid_boundary) to fluid variables [5][n]. */
+int vlasov_fluid_from_moments(const double* mom10_dev, double m, double* U5_dev, long n, void* stream);
+/* eq. (8): fluid variables [5][n] to what vlasov_set_boundary takes, [5][n] = n, bulk velocity, pressure. */
+int vlasov_fluid_to_boundary(const double* U5_dev, double m, double* fluid5_dev, long n, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,9 @@ STAGE_X1, STAGE_V, STAGE_X2, STAGE_GHOST, STAGE_MOMENTS, STAGE_ALL = 1, 2, 4, 8,
 EXPORTS = ["vlasov_scratch_bytes", "vlasov_init", "vlasov_set_boundary", "vlasov_step", "vlasov_step_host",
            "vlasov_moments", "vlasov_current", "vlasov_maxwell", "vlasov_touch", "vlasov_set_option", "vlasov_check",
            "vlasov_launch_count", "vlasov_free", "vlasov_strerror", "vlasov_cycle", "vlasov_cycle_host",
-           "vlasov_timing_enable", "vlasov_timing_read", "vlasov_fluid_boundary_mark", "vlasov_fluid_boundary"]
+           "vlasov_timing_enable", "vlasov_timing_read", "vlasov_fluid_boundary_mark", "vlasov_fluid_boundary",
+           "vlasov_fluid_scratch_bytes", "vlasov_fluid_step", "vlasov_fluid_from_moments", "vlasov_fluid_to_boundary"]
+FLUID_BC_PERIODIC, FLUID_BC_WALL, FLUID_BC_COUPLED = 0, 1, 2
 OPT_FUSE_XY = 1
 OPT_FUSE_MOMENTS = 2
 KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy", "sweep_yx",
@@ -36,6 +38,12 @@ class vlasov_config(C.Structure):
                 ("lx", C.c_double), ("ly", C.c_double), ("bc_y_lo", C.c_int32), ("bc_y_hi", C.c_int32),
                 ("order", C.c_int32), ("limiter", C.c_int32), ("fields_yee", C.c_int32), ("reserved", C.c_int32),
                 ("c", C.c_double), ("mu0", C.c_double), ("stream", C.c_void_p)]
+
+
+class vlasov_fluid_config(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nspecies", C.c_int32), ("bc_y_lo", C.c_int32),
+                ("bc_y_hi", C.c_int32), ("reserved", C.c_int32), ("dx", C.c_double), ("dy", C.c_double),
+                ("q", C.c_double * 8), ("m", C.c_double * 8), ("stream", C.c_void_p)]
 
 
 class VlasovError(RuntimeError):
@@ -97,6 +105,14 @@ def lib():
         L.vlasov_free.argtypes = [vp]
         L.vlasov_strerror.restype = C.c_char_p
         L.vlasov_strerror.argtypes = [C.c_int]
+        L.vlasov_fluid_scratch_bytes.restype = C.c_size_t
+        L.vlasov_fluid_scratch_bytes.argtypes = [C.POINTER(vlasov_fluid_config)]
+        L.vlasov_fluid_step.restype = C.c_int
+        L.vlasov_fluid_step.argtypes = [C.POINTER(vlasov_fluid_config), C.c_double, dp, dp, dp, dp, dp, vp, C.c_size_t]
+        L.vlasov_fluid_from_moments.restype = C.c_int
+        L.vlasov_fluid_from_moments.argtypes = [dp, C.c_double, dp, C.c_long, vp]
+        L.vlasov_fluid_to_boundary.restype = C.c_int
+        L.vlasov_fluid_to_boundary.argtypes = [dp, C.c_double, dp, C.c_long, vp]
         _lib = L
     return _lib
 
@@ -254,3 +270,43 @@ def context_for(workload, f_list, order=ORDER_XVX, limiter=1, stream=None):
                       workload.bc_y_lo, workload.bc_y_hi, order=order, limiter=limiter,
                       fields_yee=workload.fields_yee, c=workload.c, mu0=workload.mu0, stream=stream)
     return Context(cfg, make_species(workload.species), f_list)
+
+
+class FluidBlock:
+    """Arguments of vlasov_fluid_step for one fluid block (marshalling only).  U: torch cuda float64
+    [nspecies, 5, ny + 4, nx]."""
+
+    def __init__(self, nx, ny, dx, dy, q, m, bc_y_lo, bc_y_hi, stream=None):
+        import torch
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        cfg = vlasov_fluid_config()
+        cfg.nx, cfg.ny, cfg.nspecies = int(nx), int(ny), len(q)
+        cfg.bc_y_lo, cfg.bc_y_hi, cfg.reserved = int(bc_y_lo), int(bc_y_hi), 0
+        cfg.dx, cfg.dy = float(dx), float(dy)
+        for s in range(len(q)):
+            cfg.q[s], cfg.m[s] = float(q[s]), float(m[s])
+        cfg.stream = stream
+        self.cfg = cfg
+        nbytes = int(lib().vlasov_fluid_scratch_bytes(C.byref(cfg)))
+        if nbytes == 0:
+            raise VlasovError(EINVAL, "vlasov_fluid_scratch_bytes")
+        self.scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+
+    def vlasov_fluid_step(self, dt, U, E, B, ghost_lo=None, ghost_hi=None):
+        _chk(lib().vlasov_fluid_step(C.byref(self.cfg), float(dt), _ptr(U), _ptr(E), _ptr(B), _ptr(ghost_lo), _ptr(ghost_hi),
+                                     C.c_void_p(self.scratch.data_ptr()), C.c_size_t(self.scratch.numel())), "vlasov_fluid_step")
+
+
+def vlasov_fluid_from_moments(mom10, m, U5, stream=None):
+    import torch
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _chk(lib().vlasov_fluid_from_moments(_ptr(mom10), float(m), _ptr(U5), C.c_long(mom10.numel() // 10), C.c_void_p(st)),
+         "vlasov_fluid_from_moments")
+
+
+def vlasov_fluid_to_boundary(U5, m, fluid5, stream=None):
+    import torch
+    st = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    _chk(lib().vlasov_fluid_to_boundary(_ptr(U5), float(m), _ptr(fluid5), C.c_long(U5.numel() // 5), C.c_void_p(st)),
+         "vlasov_fluid_to_boundary")

@@ -10,7 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvlasov_b200.so")
-SOURCES = ["api.cu", "sweep_space.cu", "sweep_space_fused.cu", "sweep_velocity.cu", "moments.cu", "ghost_maxwell.cu"]
+SOURCES = ["api.cu", "sweep_space.cu", "sweep_space_fused.cu", "sweep_velocity.cu", "moments.cu", "ghost_maxwell.cu", "fluid.cu"]
 HEADERS = ["vlasov_internal.cuh", "tma.cuh", os.path.join("..", "..", "include", "vlasov.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]

@@ -273,3 +273,28 @@ def band_fluid_state(w: Workload, s: int, side: int, step_index: int) -> np.ndar
             xi = hash_noise(w.seed, 1000 + 100 * s + 10 * side + k, (step_index * g + l) * w.nx, w.nx)
             out[k, l, :] = base[k] * (1.0 + 0.01 * xi)
     return out
+
+
+def band_fluid_block(w: Workload, nyf: int, side: int):
+    """A five-moment fluid block of nyf rows below (side 0) or above (side 1) the kinetic band of workload w, same dx, dy
+    (the fluid region of the coupled set-up): the Harris-sheet moments per species as conserved variables
+    U[ns][5][nyf + 4][nx] = rho, momentum density (3), energy density (eqs. 2-4, 8; two ghost rows per side), and the
+    fields E, B [3][nyf + 4][nx] at the cell centres."""
+    import copy
+    wf = copy.deepcopy(w)
+    wf.ny, wf.nghost_y, wf.fields_yee = nyf, 2, 0
+    wf.ly = nyf * w.dy
+    wf.y0 = w.y0 - nyf * w.dy if side == 0 else w.y0 + w.ny * w.dy
+    wf.ly_domain = getattr(w, "ly_domain", w.ly)
+    E, B = gem_fields(wf)
+    yc = wf.y_centres_g()
+    U = np.zeros((len(w.species), 5, nyf + 4, w.nx))
+    for s, sp in enumerate(w.species):
+        sh = harris_density(yc)[:, None] + 0 * np.arange(w.nx)[None, :]
+        n = sh + GEM_NB
+        T = sp.m * sp.vth ** 2
+        uz = sh * sp.drift_z / n
+        U[s, 0] = sp.m * n
+        U[s, 3] = sp.m * n * uz
+        U[s, 4] = 1.5 * n * T + 0.5 * sp.m * n * uz ** 2
+    return U, E, B
