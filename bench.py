@@ -252,6 +252,54 @@ def gpu_arm(args):
         fluid = [[[torch.from_numpy(inputs.band_fluid_state(w, s, side, k)).to(device) for side in (0, 1)]
                   for s in range(ns)] for k in range(nstate)]
     step_no = [0]
+    live = None
+    if fluid is not None and args.fluid == "live":
+        # the fluid region of the coupled set-up as two live five-moment blocks (rest of the 128-row domain), fields of
+        # the fluid blocks held at their initial values (the Maxwell solve of this bench covers the band)
+        nyf = (round(w.ly_domain / w.dy) - w.ny) // 2
+        live = {"nyf": nyf, "U": [], "E": [], "B": [], "blk": [], "q": [sp.q for sp in w.species], "m": [sp.m for sp in w.species],
+                "b5": [[torch.empty((5, w.nghost_y, w.nx), dtype=torch.float64, device=device) for _ in (0, 1)] for _ in range(ns)],
+                "mb": torch.empty((10, w.nghost_y, w.nx), dtype=torch.float64, device=device),
+                "gh": [torch.zeros((3, ns, 5, 2, w.nx), dtype=torch.float64, device=device) for _ in (0, 1)]}
+        for side in (0, 1):
+            U0, Ef, Bf = inputs.band_fluid_block(w, nyf, side)
+            live["U"].append(torch.from_numpy(U0).to(device))
+            live["E"].append(torch.from_numpy(Ef).to(device)); live["B"].append(torch.from_numpy(Bf).to(device))
+            live["blk"].append(binding.FluidBlock(w.nx, nyf, w.dx, w.dy, live["q"], live["m"],
+                                                  binding.FLUID_BC_WALL if side == 0 else binding.FLUID_BC_COUPLED,
+                                                  binding.FLUID_BC_COUPLED if side == 0 else binding.FLUID_BC_WALL))
+
+    def live_before():
+        """Ghost state of the band from the fluid rows next to it (section 4.2), and the mark of section 4.1."""
+        g, nyf = w.nghost_y, live["nyf"]
+        for side in (0, 1):
+            rows = slice(2 + nyf - g, 2 + nyf) if side == 0 else slice(2, 2 + g)
+            for s in range(ns):
+                tmp = live["b5"][s][side]
+                binding.vlasov_fluid_to_boundary(live["U"][side][s][:, rows].contiguous(), live["m"][s], tmp)
+                lay = torch.flip(tmp, dims=[1]).contiguous() if side == 0 else tmp      # ghost layers count outward
+                ctx.vlasov_set_boundary(s, side, inputs.BC_FLUID, lay)
+        ctx.vlasov_fluid_boundary_mark()
+
+    def live_after():
+        """Ghost rows of the fluid blocks from the band's border rows at the Runge-Kutta stage times, then the fluid steps."""
+        for side in (0, 1):
+            pick = slice(0, 2) if side == 0 else slice(1, 3)
+            for k, th in enumerate((0.0, 1.0, 0.5)):
+                for s in range(ns):
+                    ctx.vlasov_fluid_boundary(s, side, th, live["mb"])
+                    binding.vlasov_fluid_from_moments(live["mb"][:, pick].contiguous(), live["m"][s], live["gh"][side][k, s])
+            gl, gh = (None, live["gh"][0]) if side == 0 else (live["gh"][1], None)
+            live["blk"][side].vlasov_fluid_step(w.dt, live["U"][side], live["E"][side], live["B"][side], gl, gh)
+
+    def cycle():
+        if live is not None:
+            live_before()
+            ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+            live_after()
+        else:
+            set_fluid()
+            ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
 
     def set_fluid():
         if fluid is not None:
@@ -271,8 +319,7 @@ def gpu_arm(args):
     # Timed with the library's per-launch event pairs OFF.  REPS repetitions of the timed block (each EXACTLY
     # args.steps cycles between barrier + synchronize); the reported time is the median.
     for _ in range(args.warmup):
-        set_fluid()
-        ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+        cycle()
     ctx.vlasov_check()
     ctx.vlasov_timing_enable(False)
     sampler = ClockSampler(local) if rank == 0 else None
@@ -284,8 +331,7 @@ def gpu_arm(args):
         l0 = ctx.launch_count()
         ev0.record(stream)
         for _ in range(args.steps):
-            set_fluid()
-            ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+            cycle()
         ev1.record(stream)
         barrier()
         launches = ctx.launch_count() - l0
@@ -302,8 +348,7 @@ def gpu_arm(args):
     barrier()
     ev0.record(stream)
     for _ in range(args.steps):
-        set_fluid()
-        ctx.vlasov_cycle(w.dt, w.nsub, Ed, Bd)
+        cycle()
     ev1.record(stream)
     barrier()
     ms_instr = ev0.elapsed_time(ev1)
@@ -414,6 +459,7 @@ def gpu_arm(args):
         "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nghost_y": w.nghost_y,
                    "nv": list(w.species[0].nv), "species": ns, "dt": w.dt, "maxwell_nsub": w.nsub,
                    "interior_cells_per_step": cells,
+                   "fluid": (args.fluid if fluid is not None else None),
                    "order": "VXV (PAPER.md:420; moments fused into the last vy+vz pass)" if args.order == "vxv" else "XVX (eq. 22)", "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": f"inputs larger than L2: {sum(f.numel() for f in fs) * 8 / 1e9:.2f} GB of f streamed by every pass (L2 126 MB)"},
         "clocks": clocks,
@@ -467,6 +513,8 @@ def main():
     ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed block of --steps cycles (median reported)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="gem128")
+    ap.add_argument("--fluid", default="seeded", choices=["seeded", "live"],
+                    help="band workload: ghost state from seeded fluid moments (BASELINE config 4) or from two live five-moment fluid blocks")
     ap.add_argument("--order", default="xvx", choices=["xvx", "vxv"], help="Strang order of the Vlasov step (R2); xvx is the benchmark")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of oracle time for the cpu_baseline leg")

@@ -4,6 +4,9 @@ Plain fp64 CPU implementation of the Vlasov hot path of arXiv 1406.5445, written
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
 this module.  It shares nothing with paper_1406_5445_b200/ (the CUDA path) and never imports it.
 
+The five-moment fluid step of the coupling lives in oracle/fluid.py (numpy).  cycle() below composes the time-stepping
+cycle of section 4.3 from these functions (pinned by tests/test_oracle_cycle.py).
+
 Arrays are numpy float64, C-contiguous, laid out as the interface says:
   f[ny_g, nx, nvx, nvy, nvz];  E, B, J: [3, ny_g, nx];  moments: [10, ny_g, nx].
 """

@@ -11,10 +11,12 @@
 //   f[iy_g][ix][ivx][ivy][ivz], iy_g = 0..ny+2g-1 (g ghost rows per y side), fp64.
 //   fields  E,B,J : [3][ny_g][nx];  moments: [10][ny_g][nx].
 //
-// Pins (tests/test_oracle_*.py): T1..T17 of DESIGN.md.  Parts that are pinned only by
-// self-consistency ("parity unpinned"): limiter under compressive velocity
-// shifts (R6/R15d), zeroth-order ghost extrapolation (R15a), isotropic target temperature (R15c),
-// ghost-row Dirichlet reuse (R16), Yee positions (R17).
+// Pins (tests/test_oracle_*.py): T1..T17 of DESIGN.md, the VXV pins (orc_step with order = 1: T10/T11/T5/T16 under
+// that order, Landau rate under VXV), the PEC-row pins of orc_field_at_cell and orc_current, and -- for the cycle
+// composed from these functions in oracle.py -- C1, C2.  Every function here is pinned.  Readings the paper leaves
+// open and for which no outside fact exists are DECLARED DEFINITIONS: limiter under compressive
+// velocity shifts (R6/R15d), zeroth-order ghost extrapolation (R15a), isotropic target temperature (R15c), ghost-row
+// Dirichlet reuse (R16), the choice of Yee positions (R17).
 //
 // Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC vlasov_oracle.cpp -o liboracle.so
 

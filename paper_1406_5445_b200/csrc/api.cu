@@ -332,13 +332,25 @@ int vlasov_moments(vlasov_ctx* c, int species, double* mom_dev) {
 // Section 4.1: the g interior rows next to border `side`, ghost-inclusive index of the first one
 static inline int border_row0(const Geom& G, int side) { return side == 0 ? G.g : G.ny; }
 
+// Moments (+ max) of the g interior rows next to border `side` of species s into dst [11][g*nx]: taken from the kept
+// moments when the last step reduced them and f has not changed since, else reduced from f.  These launches exist only
+// because a side is coupled: they carry the ghost timing kinds.
+static int border_moments(vlasov_ctx* c, int s, int side, double* dst) {
+    const long n = (long)c->G.g * c->G.nx, ncell = (long)c->G.nyg * c->G.nx;
+    c->ghost_tag = 1;
+    int e;
+    if (c->mom_valid) e = launch_gather_rows(c, c->mom + (long)s * 11 * ncell, ncell, (long)border_row0(c->G, side) * c->G.nx, dst, n, 11);
+    else e = launch_moments(c, c->sp[s], c->sp[s].f, dst, border_row0(c->G, side), c->G.g);
+    c->ghost_tag = 0;
+    return e;
+}
+
 int vlasov_fluid_boundary_mark(vlasov_ctx* c) {
     if (!c || c->G.g < 1 || c->G.ny < c->G.g) return VLASOV_EINVAL;
     const size_t n = (size_t)c->G.g * c->G.nx;
     for (int s = 0; s < c->ns; ++s)
         for (int side = 0; side < 2; ++side) {
-            int e = launch_moments(c, c->sp[s], c->sp[s].f, c->bmark + ((size_t)(s * 2 + side) * 11) * n,
-                                   border_row0(c->G, side), c->G.g);
+            int e = border_moments(c, s, side, c->bmark + ((size_t)(s * 2 + side) * 11) * n);
             if (e) return e;
         }
     c->bmark_valid = 1;
@@ -350,9 +362,12 @@ int vlasov_fluid_boundary(vlasov_ctx* c, int species, int side, double theta, do
     if (c->G.g < 1 || c->G.ny < c->G.g || !c->bmark_valid) return VLASOV_EINVAL;
     if (((uintptr_t)out_dev) & 7) return VLASOV_EALIGN;
     const size_t n = (size_t)c->G.g * c->G.nx;
-    int e = launch_moments(c, c->sp[species], c->sp[species].f, c->bcur, border_row0(c->G, side), c->G.g);
+    int e = border_moments(c, species, side, c->bcur);
     if (e) return e;
-    return launch_lerp(c, c->bmark + ((size_t)(species * 2 + side) * 11) * n, c->bcur, theta, out_dev, (long)(10 * n));
+    c->ghost_tag = 1;
+    e = launch_lerp(c, c->bmark + ((size_t)(species * 2 + side) * 11) * n, c->bcur, theta, out_dev, (long)(10 * n));
+    c->ghost_tag = 0;
+    return e;
 }
 
 int vlasov_current(vlasov_ctx* c, double* J_dev) {

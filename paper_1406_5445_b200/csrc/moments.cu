@@ -119,6 +119,24 @@ int launch_lerp(vlasov_ctx* c, const double* a, const double* b, double theta, d
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
 
+// rows [off, off + n) of each of nk moment planes of src [nk][src_stride] -> dst [nk][n] (the border rows of the kept
+// moments: section 4.1 needs no second pass over f when the step has just reduced them)
+__global__ void gather_rows_kernel(const double* __restrict__ src, long src_stride, long off, double* __restrict__ dst, long n, int nk) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n * nk) return;
+    const long k = i / n, j = i - k * n;
+    dst[i] = src[k * src_stride + off + j];
+}
+
+int launch_gather_rows(vlasov_ctx* c, const double* src, long src_stride, long off, double* dst, long n, int nk) {
+    if (n <= 0) return VLASOV_OK;
+    {
+        Launch L(c, K_MOMENTS);
+        gather_rows_kernel<<<(unsigned)((n * nk + 255) / 256), 256, 0, c->stream>>>(src, src_stride, off, dst, n, nk);
+    }
+    return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
+}
+
 // ------------------------------------------------------------------------------------------------
 // eq. (11): j = sum_s q_s M1^(s); Yee: interpolated to the E positions of R17
 // ------------------------------------------------------------------------------------------------

@@ -157,7 +157,16 @@ constexpr int xy_default_chunk(int sp) { return sp > 0 ? 2048 / (sp > 0 ? sp : 1
 // SP > 0: nx = SP spatial cells per row, NV^3 velocity cells, KC = the launcher's chunk for that shape (one piece:
 // C = PC = KC): every stride of the kernel is a compile-time constant.  SP = 0: any shape, at run time.
 template <int XB, int LIM, int XFIRST, int SP, int NV = 32, int KC = xy_default_chunk(SP)>
-__global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant__ CUtensorMap tmap, XYParams P) {
+#ifndef VL_XY_MAXT
+#define VL_XY_MAXT 512
+#endif
+#ifndef VL_XY_MINB
+#define VL_XY_MINB 1
+#endif
+#ifndef VL_XY_CH
+#define VL_XY_CH 4
+#endif
+__global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const __grid_constant__ CUtensorMap tmap, XYParams P) {
     extern __shared__ __align__(128) unsigned char smraw[];
     constexpr long KS = (long)NV * NV * NV;
     if (SP && (P.nx != SP || P.C != KC || P.PC != KC || P.nv1 != NV || P.nv2 != NV || P.S != KS)) return;
@@ -223,7 +232,7 @@ __global__ void __launch_bounds__(512, 1) sweep_xy_kernel(const __grid_constant_
 #pragma unroll
     for (int i = 0; i < XB; ++i) { A[i] = 0.0; B[i] = 0.0; yG[i] = 0.0; }
     const int orow_shift = ypos ? 1 : 2;
-    constexpr int CH = XB < 4 ? XB : 4;
+    constexpr int CH = XB < VL_XY_CH ? XB : VL_XY_CH;
 
     // one row; PAR = parity of r + 2: rows (r-2, r-1) = (A, B) if PAR == 0 else (B, A); the new row replaces r-2
     auto row = [&](auto par, int r, int stage, unsigned phase) {
@@ -364,7 +373,7 @@ static bool pick_xy_shape(const Geom& G, const Species& s, int& xb, int& C) {
     if (G.nx % 4 == 0) xb = 4;
     const int nblk = G.nx / xb;
     C = 32;
-    auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && nblk * cc <= 512; };
+    auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && nblk * cc <= VL_XY_MAXT; };
     while (C >= 2 && !ok(C)) C >>= 1;
     if (C < 2) return false;
     if (G.nx > 256) return false;                  // TMA box limit
@@ -421,7 +430,8 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
         else if (cube == 48 && G.nx == 64 && C == 16) { if (lim) launch_xy_t<4, 1, 64, 48, 16>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64, 48, 16>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (cube == 40 && G.nx == 256 && C == 8) { if (lim) launch_xy_t<4, 1, 256, 40, 8>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 256, 40, 8>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else
-        if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        if (v32 && G.nx == 128 && C == 8) { if (lim) launch_xy_t<4, 1, 128, 32, 8>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128, 32, 8>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (v32 && G.nx == 64 && C == 32) { if (lim) launch_xy_t<4, 1, 64>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (xb == 4) { if (lim) launch_xy_t<4, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else { if (lim) launch_xy_t<1, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }

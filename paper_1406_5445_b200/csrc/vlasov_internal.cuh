@@ -119,6 +119,7 @@ int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out
 // ghost fill (a0) of one side
 int launch_ghost_fill(vlasov_ctx* c, const Species& s, double* f, int side);
 int launch_lerp(vlasov_ctx* c, const double* a, const double* b, double theta, double* out, long n);
+int launch_gather_rows(vlasov_ctx* c, const double* src, long src_stride, long off, double* dst, long n, int nk);
 int launch_current(vlasov_ctx* c, double* J);
 int launch_maxwell(vlasov_ctx* c, double dt, int nsub, double* E, double* B, const double* J, double* Bavg);
 
