@@ -244,3 +244,76 @@ def cycle(f_list, sp_list, mom_list, E, B, nx, ny, g, lx, ly, dt, nsub, c, mu0, 
     J = current(new_mom, q, fields_yee, wall)
     maxwell(E, B, J, lx / nx, ly / ny, c, mu0, dt / 2, nsub, wall)
     return new_mom
+
+
+# ------------------------------------------------------------------------------------------------
+# 3D3V (SURVEY 8(f) NEXT-4, PAPER.md:86): f[nz, ny, nx, nvx, nvy, nvz]; fields, moments [.., nz, ny, nx]
+# ------------------------------------------------------------------------------------------------
+def sweep_z(f, sp, nx, nyg, nz, dz, dts, limiter=1):
+    assert f.flags.c_contiguous and f.dtype == np.float64
+    lib().orc_sweep_z(_d(f), nx, nyg, nz, _i3(sp.nv), _d3(sp.vmin), _d3(sp.vmax), C.c_double(dz), C.c_double(dts),
+                      C.c_double(sp.f_inf), C.c_int(limiter))
+
+
+def field_at_cell3d(E, B, fields_yee, wall, ix, j, k):
+    E = _f64(E)
+    B = _f64(B)
+    _, nz, nyg, nx = E.shape
+    Ec = np.zeros(3)
+    Bc = np.zeros(3)
+    lib().orc_field_at_cell3d(_d(E), _d(B), nx, nyg, nz, C.c_int(fields_yee), C.c_int(wall), ix, j, k, _d(Ec), _d(Bc))
+    return Ec, Bc
+
+
+def moments3d(f, sp, nx, ny, nz):
+    """[10, nz, ny, nx]: the moments are local to a spatial cell."""
+    return moments(f, sp, nx, ny * nz, 0).reshape(10, nz, ny, nx)
+
+
+def current3d(mom_list, q_list, fields_yee=0, wall=0):
+    mom = _f64(np.stack(mom_list))
+    ns, _, nz, nyg, nx = mom.shape
+    q = _f64(np.array(q_list, dtype=np.float64))
+    J = np.zeros((3, nz, nyg, nx))
+    lib().orc_current3d(_d(mom), ns, _d(q), nx, nyg, nz, C.c_int(fields_yee), C.c_int(wall), _d(J))
+    return J
+
+
+def maxwell3d(E, B, J, dx, dy, dz, c, mu0, dt, nsub, wall, want_bavg=False):
+    assert E.flags.c_contiguous and B.flags.c_contiguous
+    _, nz, nyg, nx = E.shape
+    Bavg = np.zeros_like(B) if want_bavg else None
+    lib().orc_maxwell3d(_d(E), _d(B), _d(_f64(J)), nx, nyg, nz, C.c_double(dx), C.c_double(dy), C.c_double(dz),
+                        C.c_double(c), C.c_double(mu0), C.c_double(dt), C.c_int(nsub), C.c_int(wall), _d(Bavg))
+    return Bavg
+
+
+def step3d(f, sp, nx, ny, nz, lx, ly, lz, dt, E, B, fields_yee=0, limiter=1, bc_lo=BC_PERIODIC, bc_hi=BC_PERIODIC,
+           order=ORDER_XVX, stages=STAGE_ALL, want_moments=True):
+    """One full 3D3V step of one species (no ghost rows).  f updated in place.  Returns (err, moments [10,nz,ny,nx] or None)."""
+    assert f.flags.c_contiguous and f.dtype == np.float64
+    mom = np.zeros((10, nz, ny, nx)) if (want_moments and stages & STAGE_MOMENTS) else None
+    err = lib().orc_step3d(_d(f), nx, ny, nz, _i3(sp.nv), _d3(sp.vmin), _d3(sp.vmax), C.c_double(sp.q), C.c_double(sp.m),
+                           C.c_double(lx), C.c_double(ly), C.c_double(lz), C.c_double(dt), _d(_f64(E)), _d(_f64(B)),
+                           C.c_int(fields_yee), C.c_double(sp.f_inf), C.c_int(limiter), C.c_int(bc_lo), C.c_int(bc_hi),
+                           C.c_int(order), C.c_uint(stages), _d(mom))
+    return err, mom
+
+
+def cycle3d(f_list, sp_list, mom_list, E, B, nx, ny, nz, lx, ly, lz, dt, nsub, c, mu0, fields_yee=0, bc_lo=BC_PERIODIC,
+            bc_hi=BC_PERIODIC, order=ORDER_XVX, limiter=1):
+    """The cycle of section 4.3 (see cycle()) on the 3D grid."""
+    wall = 0 if bc_lo == BC_PERIODIC else 1
+    q = [sp.q for sp in sp_list]
+    J = current3d(mom_list, q, fields_yee, wall)
+    Bavg = maxwell3d(E, B, J, lx / nx, ly / ny, lz / nz, c, mu0, dt / 2, nsub, wall, want_bavg=True)
+    new_mom = []
+    for s, sp in enumerate(sp_list):
+        err, m = step3d(f_list[s], sp, nx, ny, nz, lx, ly, lz, dt, E, Bavg, fields_yee=fields_yee, limiter=limiter,
+                        bc_lo=bc_lo, bc_hi=bc_hi, order=order)
+        if err:
+            raise RuntimeError(f"oracle step error {err}")
+        new_mom.append(m)
+    J = current3d(new_mom, q, fields_yee, wall)
+    maxwell3d(E, B, J, lx / nx, ly / ny, lz / nz, c, mu0, dt / 2, nsub, wall)
+    return new_mom

@@ -562,6 +562,196 @@ int orc_step(double* f, int nx, int ny, int g, const int* nv, const double* vmin
     return err;
 }
 
+// =============================================================================================
+// 3D3V ("a generalisation to the full 3-dimensional case is straightforward"):
+// a third spatial direction z, periodic, nz cells of width dz.  Layout f[iz][iy_g][ix][ivx][ivy][ivz]; fields and
+// moments [..][nz][ny_g][nx].  The x and y sweeps act slab by slab (the 2D functions above); the z sweep is the same
+// 1D remap along z; the fields live on the 3D Yee grid (reading R24 of DESIGN.md, the standard extension of R17).
+// With nz = 1 every function below reduces to its 2D counterpart bit for bit (pinned).
+// =============================================================================================
+
+// z half-sweep T(dts * v_z d/dz), periodic: sigma = v_z[ivz] * dts / dz on every face (eqs. 38, 46/47)
+void orc_sweep_z(double* f, int nx, int nyg, int nz, const int* nv, const double* vmin, const double* vmax,
+                 double dz, double dts, double finf, int limiter) {
+    Grid G = make_grid(nx, nyg, 0, nv, vmin, vmax);
+    const long S = G.nvtot;
+    const long slab = (long)nyg * nx * S;           // stride between z neighbours
+#pragma omp parallel
+    {
+        std::vector<double> line(nz), out(nz), sig(nz + 1);
+#pragma omp for schedule(static)
+        for (long c = 0; c < (long)nyg * nx; ++c)
+            for (long v = 0; v < S; ++v) {
+                int ivz = (int)(v % nv[2]);
+                double s = vcen(G, 2, ivz) * dts / dz;
+                for (int k = 0; k <= nz; ++k) sig[k] = s;
+                double* base = f + c * S + v;
+                for (int k = 0; k < nz; ++k) line[k] = base[(long)k * slab];
+                remap_line(line.data(), nz, sig.data(), 0, finf, limiter, out.data());
+                for (int k = 0; k < nz; ++k) base[(long)k * slab] = out[k];
+            }
+    }
+}
+
+// Fields at the centre of cell (ix, j, k).  3D Yee positions (R24): cell (i,j,k) spans [i dx,(i+1)dx] x [j dy,(j+1)dy] x
+// [k dz,(k+1)dz]; Ex(i+1/2,j,k) Ey(i,j+1/2,k) Ez(i,j,k+1/2) Bx(i,j+1/2,k+1/2) By(i+1/2,j,k+1/2) Bz(i+1/2,j+1/2,k);
+// linear interpolation to the centre; x and z periodic, row j+1 beyond the array: wrap or PEC wall value 0.
+void orc_field_at_cell3d(const double* E, const double* B, int nx, int nyg, int nz, int fields_yee, int wall,
+                         int ix, int j, int k, double* Ec, double* Bc) {
+    const long P = (long)nz * nyg * nx;
+    auto at = [&](const double* A, int d, int kk, int jj, int ii) { return A[d * P + ((long)kk * nyg + jj) * nx + ii]; };
+    if (!fields_yee) {
+        for (int d = 0; d < 3; ++d) { Ec[d] = at(E, d, k, j, ix); Bc[d] = at(B, d, k, j, ix); }
+        return;
+    }
+    int ip = (ix + 1) % nx, kp = (k + 1) % nz;
+    int jp = j + 1;
+    double up = 1.0;
+    if (jp >= nyg) { jp = 0; if (wall) up = 0.0; }
+    Ec[0] = 0.25 * ((at(E, 0, k, j, ix) + up * at(E, 0, k, jp, ix)) + (at(E, 0, kp, j, ix) + up * at(E, 0, kp, jp, ix)));
+    Ec[1] = 0.25 * ((at(E, 1, k, j, ix) + at(E, 1, k, j, ip)) + (at(E, 1, kp, j, ix) + at(E, 1, kp, j, ip)));
+    Ec[2] = 0.25 * (at(E, 2, k, j, ix) + at(E, 2, k, j, ip) + up * at(E, 2, k, jp, ix) + up * at(E, 2, k, jp, ip));
+    Bc[0] = 0.5 * (at(B, 0, k, j, ix) + at(B, 0, k, j, ip));
+    Bc[1] = 0.5 * (at(B, 1, k, j, ix) + up * at(B, 1, k, jp, ix));
+    Bc[2] = 0.5 * (at(B, 2, k, j, ix) + at(B, 2, kp, j, ix));
+}
+
+int orc_vstep3d(double* f, int nx, int nyg, int nz, const int* nv, const double* vmin, const double* vmax,
+                double q, double m, double dt, const double* E, const double* B, int fields_yee,
+                int wall, double finf, int limiter) {
+    Grid G = make_grid(nx, nyg, 0, nv, vmin, vmax);
+    int err = ERR_OK;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < nyg; ++j)
+            for (int ix = 0; ix < nx; ++ix) {
+                double Ec[3], Bc[3], t[3], s[3], h[3];
+                orc_field_at_cell3d(E, B, nx, nyg, nz, fields_yee, wall, ix, j, k, Ec, Bc);
+                int e = orc_boris_coeffs(Ec, Bc, q, m, dt, t, s, h);
+                if (e) {
+#pragma omp critical
+                    err = e;
+                    continue;
+                }
+                orc_vsweeps_block(f + (((long)k * nyg + j) * nx + ix) * G.nvtot, nv, vmin, vmax, t, s, h, finf, limiter, 0);
+            }
+    return err;
+}
+
+// eq. (11) on the 3D Yee grid: J at the E positions by linear interpolation of the cell-centre currents.
+// mom: [ns][10][nz][nyg][nx].
+void orc_current3d(const double* mom, int ns, const double* q, int nx, int nyg, int nz, int fields_yee, int wall,
+                   double* J) {
+    const long P = (long)nz * nyg * nx;
+    std::vector<double> jc(3 * P, 0.0);
+    for (int s = 0; s < ns; ++s)
+        for (int d = 0; d < 3; ++d)
+            for (long c = 0; c < P; ++c) jc[d * P + c] += q[s] * mom[((long)s * 10 + 1 + d) * P + c];
+    if (!fields_yee) { std::memcpy(J, jc.data(), sizeof(double) * 3 * P); return; }
+    auto at = [&](int d, int k, int j, int i) { return jc[d * P + ((long)k * nyg + j) * nx + i]; };
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < nyg; ++j)
+            for (int i = 0; i < nx; ++i) {
+                int im = (i + nx - 1) % nx, km = (k + nz - 1) % nz;
+                int jm = j - 1;
+                double lo = 1.0;
+                if (jm < 0) { jm = nyg - 1; if (wall) lo = 0.0; }
+                const long o = ((long)k * nyg + j) * nx + i;
+                J[0 * P + o] = lo == 0.0 ? 0.0 : 0.25 * ((at(0, km, jm, i) + at(0, km, j, i)) + (at(0, k, jm, i) + at(0, k, j, i)));
+                J[1 * P + o] = 0.25 * ((at(1, km, j, im) + at(1, km, j, i)) + (at(1, k, j, im) + at(1, k, j, i)));
+                J[2 * P + o] = lo == 0.0 ? 0.0 : 0.25 * (at(2, k, jm, im) + at(2, k, jm, i) + at(2, k, j, im) + at(2, k, j, i));
+            }
+}
+
+// 3D Yee FDTD leapfrog, eqs. (9), (10): nsub sub-steps of ddt = dt/nsub, E first, then B; x, z periodic; y periodic or
+// PEC walls at the node rows j = 0 and j = nyg (E_x = E_z = 0, B_y = 0 there).
+void orc_maxwell3d(double* E, double* B, const double* J, int nx, int nyg, int nz, double dx, double dy, double dz,
+                   double c, double mu0, double dt, int nsub, int wall, double* Bavg) {
+    const long P = (long)nz * nyg * nx;
+    const double ddt = dt / nsub;
+    auto idx = [&](int d, int k, int j, int i) { return d * P + ((long)k * nyg + j) * nx + i; };
+    std::vector<double> Bold(3 * P);
+    for (int sub = 0; sub < nsub; ++sub) {
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < nyg; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    int im = (i + nx - 1) % nx, km = (k + nz - 1) % nz;
+                    int jm = j - 1;
+                    bool onwall = false;
+                    if (jm < 0) { jm = nyg - 1; onwall = wall != 0; }
+                    double curlx = (B[idx(2, k, j, i)] - B[idx(2, k, jm, i)]) / dy - (B[idx(1, k, j, i)] - B[idx(1, km, j, i)]) / dz;
+                    double curly = (B[idx(0, k, j, i)] - B[idx(0, km, j, i)]) / dz - (B[idx(2, k, j, i)] - B[idx(2, k, j, im)]) / dx;
+                    double curlz = (B[idx(1, k, j, i)] - B[idx(1, k, j, im)]) / dx - (B[idx(0, k, j, i)] - B[idx(0, k, jm, i)]) / dy;
+                    if (!onwall) E[idx(0, k, j, i)] += ddt * c * c * (curlx - mu0 * J[idx(0, k, j, i)]);
+                    else         E[idx(0, k, j, i)] = 0.0;
+                    E[idx(1, k, j, i)] += ddt * c * c * (curly - mu0 * J[idx(1, k, j, i)]);
+                    if (!onwall) E[idx(2, k, j, i)] += ddt * c * c * (curlz - mu0 * J[idx(2, k, j, i)]);
+                    else         E[idx(2, k, j, i)] = 0.0;
+                }
+        if (Bavg && sub == nsub - 1) std::memcpy(Bold.data(), B, sizeof(double) * 3 * P);
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < nyg; ++j)
+                for (int i = 0; i < nx; ++i) {
+                    int ip = (i + 1) % nx, kp = (k + 1) % nz;
+                    int jp = j + 1;
+                    double up = 1.0;
+                    if (jp >= nyg) { jp = 0; if (wall) up = 0.0; }
+                    double dEz_dy = (up * E[idx(2, k, jp, i)] - E[idx(2, k, j, i)]) / dy;
+                    double dEy_dz = (E[idx(1, kp, j, i)] - E[idx(1, k, j, i)]) / dz;
+                    double dEx_dz = (E[idx(0, kp, j, i)] - E[idx(0, k, j, i)]) / dz;
+                    double dEz_dx = (E[idx(2, k, j, ip)] - E[idx(2, k, j, i)]) / dx;
+                    double dEy_dx = (E[idx(1, k, j, ip)] - E[idx(1, k, j, i)]) / dx;
+                    double dEx_dy = (up * E[idx(0, k, jp, i)] - E[idx(0, k, j, i)]) / dy;
+                    B[idx(0, k, j, i)] -= ddt * (dEz_dy - dEy_dz);
+                    if (wall && j == 0) B[idx(1, k, j, i)] = 0.0;
+                    else                B[idx(1, k, j, i)] -= ddt * (dEx_dz - dEz_dx);
+                    B[idx(2, k, j, i)] -= ddt * (dEy_dx - dEx_dy);
+                }
+    }
+    if (Bavg) for (long q = 0; q < 3 * P; ++q) Bavg[q] = 0.5 * (Bold[q] + B[q]);
+}
+
+// Full 3D3V step of one species.  XVX (eq. 22): x/2 y/2 z/2 -- vx vy vz -- z/2 y/2 x/2 (palindrome, R3 extended);
+// VXV: v/2 -- x y z -- v/2.  y sides PERIODIC or REFLECT (no ghost rows: g = 0); stages as in orc_step.
+int orc_step3d(double* f, int nx, int ny, int nz, const int* nv, const double* vmin, const double* vmax,
+               double q, double m, double x_len, double y_len, double z_len, double dt, const double* E, const double* B,
+               int fields_yee, double finf, int limiter, int bc_lo, int bc_hi, int order, unsigned stages, double* mom) {
+    const double dx = x_len / nx, dy = y_len / ny, dz = z_len / nz;
+    const int wall = (bc_lo == BC_PERIODIC) ? 0 : 1;
+    Grid G = make_grid(nx, ny, 0, nv, vmin, vmax);
+    const long slab = (long)ny * nx * G.nvtot;
+    int err = ERR_OK, e;
+    auto space = [&](double dts, bool forward) {
+        if (forward) {
+            for (int k = 0; k < nz; ++k) {
+                orc_sweep_x(f + k * slab, nx, ny, 0, nv, vmin, vmax, dx, dts, finf, limiter);
+                e = orc_sweep_y(f + k * slab, nx, ny, 0, nv, vmin, vmax, dy, dts, finf, limiter, bc_lo, bc_hi); if (e) err = e;
+            }
+            orc_sweep_z(f, nx, ny, nz, nv, vmin, vmax, dz, dts, finf, limiter);
+        } else {
+            orc_sweep_z(f, nx, ny, nz, nv, vmin, vmax, dz, dts, finf, limiter);
+            for (int k = 0; k < nz; ++k) {
+                e = orc_sweep_y(f + k * slab, nx, ny, 0, nv, vmin, vmax, dy, dts, finf, limiter, bc_lo, bc_hi); if (e) err = e;
+                orc_sweep_x(f + k * slab, nx, ny, 0, nv, vmin, vmax, dx, dts, finf, limiter);
+            }
+        }
+    };
+    auto velocity = [&](double dtv) {
+        e = orc_vstep3d(f, nx, ny, nz, nv, vmin, vmax, q, m, dtv, E, B, fields_yee, wall, finf, limiter); if (e) err = e;
+    };
+    if (order == 0) {
+        if (stages & 1u) space(dt / 2.0, true);
+        if (stages & 2u) velocity(dt);
+        if (stages & 4u) space(dt / 2.0, false);
+    } else {
+        if (stages & 1u) velocity(dt / 2.0);
+        if (stages & 2u) space(dt, true);
+        if (stages & 4u) velocity(dt / 2.0);
+    }
+    if ((stages & 16u) && mom) orc_moments(f, nx, ny * nz, 0, nv, vmin, vmax, mom);
+    return err;
+}
+
 int orc_num_threads(void) {
     int n = 1;
 #ifdef _OPENMP
