@@ -19,6 +19,8 @@
  *   f_s      [ny_g][nx][nvx][nvy][nvz]   cell averages (R1), velocity fastest, ny_g = ny + 2 nghost_y
  *   E, B, J  [3][ny_g][nx]
  *   moments  [10][ny_g][nx] = M0, M1x, M1y, M1z, M2xx, M2yy, M2zz, M2xy, M2xz, M2yz
+ *   3D3V (cfg.nz > 1): f_s [nz][ny][nx][nvx][nvy][nvz], E, B, J [3][nz][ny][nx], moments [10][nz][ny][nx]; the step
+ *   is x/2 y/2 z/2 - vx vy vz - z/2 y/2 x/2 (XVX) or v/2 - x y z - v/2 (VXV); fields on the 3D Yee grid (R24)
  *   fluid5   [5][nghost_y][nx] = n, ux, uy, uz, p; ghost layer index counted OUTWARD from the edge
  */
 #ifndef VLASOV_B200_H
@@ -75,9 +77,11 @@ typedef struct {
     int32_t bc_y_lo, bc_y_hi;
     int32_t order;        /* VLASOV_ORDER_* */
     int32_t limiter;      /* 1 = eqs. (43),(44); 0 = eps == 1 (unlimited third order) */
-    int32_t fields_yee;   /* 0: E,B,J cell-centred; 1: 2D Yee positions of R17 */
-    int32_t reserved;
+    int32_t fields_yee;   /* 0: E,B,J cell-centred; 1: Yee positions of R17 / R24 */
+    int32_t nz;           /* 3D3V (NEXT-4): cells along z, periodic; 0 or 1 = the 2D3V path.  nz > 1 needs
+                             nghost_y == 0 (no FLUID sides) and lz > 0; every array gains a slowest index iz */
     double c, mu0;        /* Maxwell constants, eqs. (9),(10) PAPER.md:68-71 */
+    double lz;            /* extent along z: dz = lz/nz (ignored for nz <= 1) */
     void* stream;         /* cudaStream_t; NULL = legacy default stream */
 } vlasov_config;
 
@@ -168,6 +172,7 @@ enum {
     /* launches that only exist because a side is FLUID (config 4's "ghost-fill share of step time"): the ghost fill's
      * velocity remaps and edge-row moments (section 4.2), and the x sweeps of the ghost rows beside a fused stage */
     VLASOV_KIND_GHOST_VSWEEP_X, VLASOV_KIND_GHOST_VSWEEP_YZ, VLASOV_KIND_GHOST_MOMENTS, VLASOV_KIND_GHOST_SWEEP_X,
+    VLASOV_KIND_SWEEP_Z /* 3D3V: the third spatial sweep */,
     VLASOV_KIND_COUNT
 };
 int vlasov_timing_enable(vlasov_ctx* ctx, int on);

@@ -25,7 +25,7 @@ FLUID_BC_PERIODIC, FLUID_BC_WALL, FLUID_BC_COUPLED = 0, 1, 2
 OPT_FUSE_XY = 1
 OPT_FUSE_MOMENTS = 2
 KINDS = ["sweep_x", "sweep_y", "table", "vsweep_x", "vsweep_yz", "moments", "ghost_table", "current", "maxwell", "sweep_xy", "sweep_yx",
-         "ghost_vsweep_x", "ghost_vsweep_yz", "ghost_moments", "ghost_sweep_x"]
+         "ghost_vsweep_x", "ghost_vsweep_yz", "ghost_moments", "ghost_sweep_x", "sweep_z"]
 
 
 class vlasov_species(C.Structure):
@@ -36,8 +36,8 @@ class vlasov_species(C.Structure):
 class vlasov_config(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nghost_y", C.c_int32), ("nspecies", C.c_int32),
                 ("lx", C.c_double), ("ly", C.c_double), ("bc_y_lo", C.c_int32), ("bc_y_hi", C.c_int32),
-                ("order", C.c_int32), ("limiter", C.c_int32), ("fields_yee", C.c_int32), ("reserved", C.c_int32),
-                ("c", C.c_double), ("mu0", C.c_double), ("stream", C.c_void_p)]
+                ("order", C.c_int32), ("limiter", C.c_int32), ("fields_yee", C.c_int32), ("nz", C.c_int32),
+                ("c", C.c_double), ("mu0", C.c_double), ("lz", C.c_double), ("stream", C.c_void_p)]
 
 
 class vlasov_fluid_config(C.Structure):
@@ -136,13 +136,13 @@ def _ptr(t):
 
 
 def make_config(nx, ny, nghost_y, nspecies, lx, ly, bc_y_lo, bc_y_hi, order=ORDER_XVX, limiter=1, fields_yee=0,
-                c=1.0, mu0=1.0, stream=0):
+                c=1.0, mu0=1.0, stream=0, nz=1, lz=1.0):
     cfg = vlasov_config()
     cfg.nx, cfg.ny, cfg.nghost_y, cfg.nspecies = nx, ny, nghost_y, nspecies
     cfg.lx, cfg.ly = lx, ly
     cfg.bc_y_lo, cfg.bc_y_hi = bc_y_lo, bc_y_hi
-    cfg.order, cfg.limiter, cfg.fields_yee, cfg.reserved = order, limiter, fields_yee, 0
-    cfg.c, cfg.mu0 = c, mu0
+    cfg.order, cfg.limiter, cfg.fields_yee, cfg.nz = order, limiter, fields_yee, int(nz)
+    cfg.c, cfg.mu0, cfg.lz = c, mu0, float(lz)
     cfg.stream = stream
     return cfg
 
@@ -166,7 +166,8 @@ def vlasov_scratch_bytes(cfg, species_arr):
 
 
 class Context:
-    """Owns a vlasov_ctx*.  f_list: torch cuda float64 tensors [ny_g, nx, nvx, nvy, nvz] (kept alive here)."""
+    """Owns a vlasov_ctx*.  f_list: torch cuda float64 tensors [ny_g, nx, nvx, nvy, nvz] ([nz, ny, nx, ...] for 3D3V),
+    kept alive here."""
 
     def __init__(self, cfg, species_arr, f_list, scratch=None):
         import torch
@@ -268,7 +269,8 @@ def context_for(workload, f_list, order=ORDER_XVX, limiter=1, stream=None):
         stream = torch.cuda.current_stream().cuda_stream
     cfg = make_config(workload.nx, workload.ny, workload.nghost_y, len(workload.species), workload.lx, workload.ly,
                       workload.bc_y_lo, workload.bc_y_hi, order=order, limiter=limiter,
-                      fields_yee=workload.fields_yee, c=workload.c, mu0=workload.mu0, stream=stream)
+                      fields_yee=workload.fields_yee, c=workload.c, mu0=workload.mu0, stream=stream,
+                      nz=getattr(workload, "nz", 1), lz=getattr(workload, "lz", 1.0))
     return Context(cfg, make_species(workload.species), f_list)
 
 

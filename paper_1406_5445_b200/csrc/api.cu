@@ -18,7 +18,7 @@ bool carve(const vlasov_config* cfg, const vlasov_species* sp, Carve& C) {
     if (!cfg || !sp) return false;
     if (cfg->nx <= 0 || cfg->ny <= 0 || cfg->nghost_y < 0 || cfg->nspecies <= 0 || cfg->nspecies > MAX_SPECIES) return false;
     const size_t nyg = (size_t)cfg->ny + 2 * (size_t)cfg->nghost_y;
-    const size_t ncell = nyg * cfg->nx;
+    const size_t ncell = nyg * cfg->nx * (size_t)(cfg->nz > 1 ? cfg->nz : 1);
     size_t maxS = 0;
     for (int s = 0; s < cfg->nspecies; ++s) {
         if (sp[s].nv[0] <= 0 || sp[s].nv[1] <= 0 || sp[s].nv[2] <= 0 || (sp[s].nv[2] & 1)) return false;
@@ -56,9 +56,11 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
     // stage is ONE pass cur -> other, so the buffers swap roles; an odd number of fused stages in one call
     // is settled by a copy back into the caller's buffer at the end.
     double* cur = s.f;
-    auto space = [&](double dts, bool x_first) -> int {
+    auto other_of = [&](double* p) { return p == s.f ? c->pong : s.f; };
+    // x and y half sweeps of one spatial stage (every z slab), src = cur; leaves the result in cur
+    auto space_xy = [&](double dts, bool x_first) -> int {
         int r;
-        double* other = cur == s.f ? c->pong : s.f;
+        double* other = other_of(cur);
         if (c->fuse_xy && fused_xy_applicable(c, s, dts)) {
             r = launch_sweep_xy(c, s, cur, other, dts, x_first ? 1 : 0); if (r) return r;
             if (G.g > 0) {      // x sweeps update ghost rows too, y sweeps never do (R16)
@@ -78,6 +80,20 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         r = launch_sweep_y(c, s, cur, other, dts); if (r) return r;
         return launch_sweep_x(c, s, other, cur, dts);
     };
+    auto space_z = [&](double dts) -> int {          // 3D3V: the third spatial sweep, out of place
+        if (G.nz <= 1) return VLASOV_OK;
+        double* other = other_of(cur);
+        int r = launch_sweep_z(c, s, cur, other, dts); if (r) return r;
+        cur = other;
+        return VLASOV_OK;
+    };
+    // forward: x y z (before the velocity step); backward: z y x (palindrome, R3)
+    auto space = [&](double dts, bool forward) -> int {
+        int r;
+        if (forward) { r = space_xy(dts, true); if (r) return r; return space_z(dts); }
+        r = space_z(dts); if (r) return r;
+        return space_xy(dts, false);
+    };
     bool mom_done = false;
     // flips_after: how many fused (one pass, buffer-swapping) spatial stages still follow in this call.  The vx sweep
     // can read one buffer and write the other, so the velocity step is where f changes sides for free: it leaves f
@@ -87,12 +103,15 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         double* target = (flips_after & 1) ? c->pong : s.f;
         // with_moments (the last pass of a VXV step): the moments of the final f may be reduced by the vy+vz kernel
         // itself.  All rows, ghost rows too (R16).
-        double* mo = with_moments && c->fuse_mom && target == s.f ? c->mom + (long)si * 11 * ((long)G.nyg * G.nx) : nullptr;
-        r = launch_vsweeps(c, s, target, 0, G.nyg, false, mo, &mom_done, cur);
+        double* mo = with_moments && c->fuse_mom && target == s.f ? c->mom + (long)si * 11 * ((long)G.nrows * G.nx) : nullptr;
+        r = launch_vsweeps(c, s, target, 0, G.nrows, false, mo, &mom_done, cur);
         cur = target;
         return r;
     };
-    auto flips = [&](bool requested, double dts) { return requested && c->fuse_xy && fused_xy_applicable(c, s, dts) ? 1 : 0; };
+    // buffer changes of one spatial stage: the fused x,y pass (one) and the z sweep (one)
+    auto flips = [&](bool requested, double dts) {
+        return !requested ? 0 : (c->fuse_xy && fused_xy_applicable(c, s, dts) ? 1 : 0) + (G.nz > 1 ? 1 : 0);
+    };
     if (c->order == VLASOV_ORDER_XVX) {
         if (stages & VLASOV_STAGE_X1) { e = space(dt / 2.0, true); if (e) return e; }
         if (stages & VLASOV_STAGE_V) { e = velocity(dt, flips((stages & VLASOV_STAGE_X2) != 0, dt / 2.0)); if (e) return e; }
@@ -103,21 +122,21 @@ int species_step(vlasov_ctx* c, int si, double dt, const double* E, const double
         if (stages & VLASOV_STAGE_X2) { e = velocity(dt / 2.0, 0, (stages & VLASOV_STAGE_MOMENTS) != 0); if (e) return e; }
     }
     if (cur != s.f) {
-        VL_CUDA_OK(cudaMemcpyAsync(s.f, cur, (size_t)G.nyg * G.nx * s.nvtot * 8, cudaMemcpyDeviceToDevice, c->stream));
+        VL_CUDA_OK(cudaMemcpyAsync(s.f, cur, (size_t)G.nrows * G.nx * s.nvtot * 8, cudaMemcpyDeviceToDevice, c->stream));
         c->launches++;
     }
     if ((stages & VLASOV_STAGE_MOMENTS) && !mom_done) {
-        const long ncell = (long)G.nyg * G.nx;
-        e = launch_moments(c, s, s.f, c->mom + (long)si * 11 * ncell, 0, G.nyg); if (e) return e;
+        const long ncell = (long)G.nrows * G.nx;
+        e = launch_moments(c, s, s.f, c->mom + (long)si * 11 * ncell, 0, G.nrows); if (e) return e;
     }
     return VLASOV_OK;
 }
 
 int ensure_moments(vlasov_ctx* c) {
     if (c->mom_valid) return VLASOV_OK;
-    const long ncell = (long)c->G.nyg * c->G.nx;
+    const long ncell = (long)c->G.nrows * c->G.nx;
     for (int s = 0; s < c->ns; ++s) {
-        int e = launch_moments(c, c->sp[s], c->sp[s].f, c->mom + (long)s * 11 * ncell, 0, c->G.nyg);
+        int e = launch_moments(c, c->sp[s], c->sp[s].f, c->mom + (long)s * 11 * ncell, 0, c->G.nrows);
         if (e) return e;
     }
     c->mom_valid = 1;
@@ -144,6 +163,8 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     if ((cfg->bc_y_lo == VLASOV_BC_PERIODIC) != (cfg->bc_y_hi == VLASOV_BC_PERIODIC)) return VLASOV_EINVAL;
     if ((cfg->bc_y_lo == VLASOV_BC_FLUID || cfg->bc_y_hi == VLASOV_BC_FLUID) && cfg->nghost_y < 1) return VLASOV_EINVAL;
     if (cfg->order != VLASOV_ORDER_XVX && cfg->order != VLASOV_ORDER_VXV) return VLASOV_EINVAL;
+    if (cfg->nz < 0) return VLASOV_EINVAL;
+    if (cfg->nz > 1 && (cfg->nghost_y != 0 || !(cfg->lz > 0.0))) return VLASOV_EINVAL;       // 3D3V: no ghost rows
     if (((uintptr_t)scratch_dev) & 127) return VLASOV_EALIGN;
     for (int s = 0; s < cfg->nspecies; ++s) {
         if (!f_dev[s]) return VLASOV_EINVAL;
@@ -164,6 +185,9 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     if (!c) return VLASOV_ECUDA;
     c->G.nx = cfg->nx; c->G.ny = cfg->ny; c->G.g = cfg->nghost_y; c->G.nyg = cfg->ny + 2 * cfg->nghost_y;
     c->G.dx = cfg->lx / cfg->nx; c->G.dy = cfg->ly / cfg->ny;
+    c->G.nz = cfg->nz > 1 ? cfg->nz : 1;
+    c->G.nrows = c->G.nz * c->G.nyg;
+    c->G.dz = c->G.nz > 1 ? cfg->lz / cfg->nz : 1.0;
     c->G.bc_lo = cfg->bc_y_lo; c->G.bc_hi = cfg->bc_y_hi;
     c->G.limiter = cfg->limiter ? 1 : 0; c->G.fields_yee = cfg->fields_yee ? 1 : 0;
     c->G.wall = cfg->bc_y_lo == VLASOV_BC_PERIODIC ? 0 : 1;
@@ -239,7 +263,7 @@ int vlasov_step(vlasov_ctx* c, double dt, const double* E_dev, const double* B_d
 int vlasov_step_host(vlasov_ctx* c, double dt, const double* E_host, const double* B_host, uint32_t stages,
                      double* mom_host) {
     if (!c || !E_host || !B_host) return VLASOV_EINVAL;
-    const size_t ncell = (size_t)c->G.nyg * c->G.nx;
+    const size_t ncell = (size_t)c->G.nrows * c->G.nx;
     double* Ed = c->fields_stage;
     double* Bd = c->fields_stage + 3 * ncell;
     VL_CUDA_OK(cudaMemcpyAsync(Ed, E_host, 3 * ncell * 8, cudaMemcpyHostToDevice, c->stream));
@@ -270,7 +294,7 @@ int vlasov_cycle(vlasov_ctx* c, double dt, int nsub, double* E_dev, double* B_de
 
 int vlasov_cycle_host(vlasov_ctx* c, double dt, int nsub, double* E_host, double* B_host, double* mom_host) {
     if (!c || !E_host || !B_host) return VLASOV_EINVAL;
-    const size_t ncell = (size_t)c->G.nyg * c->G.nx;
+    const size_t ncell = (size_t)c->G.nrows * c->G.nx;
     double* Ed = c->fields_stage;
     double* Bd = c->fields_stage + 3 * ncell;
     VL_CUDA_OK(cudaMemcpyAsync(Ed, E_host, 3 * ncell * 8, cudaMemcpyHostToDevice, c->stream));
@@ -323,7 +347,7 @@ int vlasov_moments(vlasov_ctx* c, int species, double* mom_dev) {
     if (((uintptr_t)mom_dev) & 7) return VLASOV_EALIGN;
     int e = ensure_moments(c);
     if (e) return e;
-    const size_t ncell = (size_t)c->G.nyg * c->G.nx;
+    const size_t ncell = (size_t)c->G.nrows * c->G.nx;
     VL_CUDA_OK(cudaMemcpyAsync(mom_dev, c->mom + (size_t)species * 11 * ncell, 10 * ncell * 8,
                                cudaMemcpyDeviceToDevice, c->stream));
     return VLASOV_OK;
@@ -346,7 +370,7 @@ static int border_moments(vlasov_ctx* c, int s, int side, double* dst) {
 }
 
 int vlasov_fluid_boundary_mark(vlasov_ctx* c) {
-    if (!c || c->G.g < 1 || c->G.ny < c->G.g) return VLASOV_EINVAL;
+    if (!c || c->G.g < 1 || c->G.ny < c->G.g || c->G.nz > 1) return VLASOV_EINVAL;
     const size_t n = (size_t)c->G.g * c->G.nx;
     for (int s = 0; s < c->ns; ++s)
         for (int side = 0; side < 2; ++side) {

@@ -96,53 +96,58 @@ struct MaxParams {
     double* __restrict__ B;
     const double* __restrict__ J;
     double* __restrict__ Bavg;
-    int nx, nyg, wall;
-    double dx, dy, c, mu0, ddt;
+    int nx, nyg, nz, wall;
+    double dx, dy, dz, c, mu0, ddt;
     int last;
 };
 
-// E += ddt c^2 (curl B - mu0 J), eq. (10)
+// E += ddt c^2 (curl B - mu0 J), eq. (10), on the Yee grid (R17; 3D: R24).  With nz = 1 every z difference
+// is x - x = 0 and the update is the 2D one bit for bit.
 __global__ void maxwell_E_kernel(MaxParams P) {
     const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     if (cell >= ncell) return;
-    const int j = cell / P.nx, i = cell % P.nx;
+    const int i = cell % P.nx, j = (cell / P.nx) % P.nyg, k = cell / (P.nx * P.nyg);
     const long PL = ncell;
-    const int im = (i + P.nx - 1) % P.nx;
+    const int im = (i + P.nx - 1) % P.nx, km = (k + P.nz - 1) % P.nz;
     int jm = j - 1;
     bool onwall = false;
     if (jm < 0) { jm = P.nyg - 1; onwall = P.wall != 0; }
     const double* B = P.B;
-    const long c0 = cell, cjm = (long)jm * P.nx + i, cim = (long)j * P.nx + im;
-    const double curlx = (B[2 * PL + c0] - B[2 * PL + cjm]) / P.dy;
-    const double curly = -(B[2 * PL + c0] - B[2 * PL + cim]) / P.dx;
+    const long c0 = cell, cjm = ((long)k * P.nyg + jm) * P.nx + i, cim = ((long)k * P.nyg + j) * P.nx + im,
+               ckm = ((long)km * P.nyg + j) * P.nx + i;
+    const double curlx = (B[2 * PL + c0] - B[2 * PL + cjm]) / P.dy - (B[1 * PL + c0] - B[1 * PL + ckm]) / P.dz;
+    const double curly = (B[0 * PL + c0] - B[0 * PL + ckm]) / P.dz - (B[2 * PL + c0] - B[2 * PL + cim]) / P.dx;
     const double curlz = (B[1 * PL + c0] - B[1 * PL + cim]) / P.dx - (B[0 * PL + c0] - B[0 * PL + cjm]) / P.dy;
-    const double k = P.ddt * P.c * P.c;
-    P.E[0 * PL + c0] = onwall ? 0.0 : P.E[0 * PL + c0] + k * (curlx - P.mu0 * P.J[0 * PL + c0]);
-    P.E[1 * PL + c0] = P.E[1 * PL + c0] + k * (curly - P.mu0 * P.J[1 * PL + c0]);
-    P.E[2 * PL + c0] = onwall ? 0.0 : P.E[2 * PL + c0] + k * (curlz - P.mu0 * P.J[2 * PL + c0]);
+    const double kk = P.ddt * P.c * P.c;
+    P.E[0 * PL + c0] = onwall ? 0.0 : P.E[0 * PL + c0] + kk * (curlx - P.mu0 * P.J[0 * PL + c0]);
+    P.E[1 * PL + c0] = P.E[1 * PL + c0] + kk * (curly - P.mu0 * P.J[1 * PL + c0]);
+    P.E[2 * PL + c0] = onwall ? 0.0 : P.E[2 * PL + c0] + kk * (curlz - P.mu0 * P.J[2 * PL + c0]);
 }
 
 // B -= ddt curl E, eq. (9); on the last sub-step also Bavg = (B_old + B_new)/2
 __global__ void maxwell_B_kernel(MaxParams P) {
     const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     if (cell >= ncell) return;
-    const int j = cell / P.nx, i = cell % P.nx;
+    const int i = cell % P.nx, j = (cell / P.nx) % P.nyg, k = cell / (P.nx * P.nyg);
     const long PL = ncell;
-    const int ip = (i + 1) % P.nx;
+    const int ip = (i + 1) % P.nx, kp = (k + 1) % P.nz;
     int jp = j + 1;
     double up = 1.0;
     if (jp >= P.nyg) { jp = 0; if (P.wall) up = 0.0; }
     const double* E = P.E;
-    const long c0 = cell, cjp = (long)jp * P.nx + i, cip = (long)j * P.nx + ip;
+    const long c0 = cell, cjp = ((long)k * P.nyg + jp) * P.nx + i, cip = ((long)k * P.nyg + j) * P.nx + ip,
+               ckp = ((long)kp * P.nyg + j) * P.nx + i;
     const double dEz_dy = (up * E[2 * PL + cjp] - E[2 * PL + c0]) / P.dy;
+    const double dEy_dz = (E[1 * PL + ckp] - E[1 * PL + c0]) / P.dz;
+    const double dEx_dz = (E[0 * PL + ckp] - E[0 * PL + c0]) / P.dz;
     const double dEz_dx = (E[2 * PL + cip] - E[2 * PL + c0]) / P.dx;
     const double dEy_dx = (E[1 * PL + cip] - E[1 * PL + c0]) / P.dx;
     const double dEx_dy = (up * E[0 * PL + cjp] - E[0 * PL + c0]) / P.dy;
     const double b0 = P.B[0 * PL + c0], b1 = P.B[1 * PL + c0], b2 = P.B[2 * PL + c0];
-    const double n0 = b0 - P.ddt * dEz_dy;
-    const double n1 = (P.wall && j == 0) ? 0.0 : b1 + P.ddt * dEz_dx;
+    const double n0 = b0 - P.ddt * (dEz_dy - dEy_dz);
+    const double n1 = (P.wall && j == 0) ? 0.0 : b1 - P.ddt * (dEx_dz - dEz_dx);
     const double n2 = b2 - P.ddt * (dEy_dx - dEx_dy);
     P.B[0 * PL + c0] = n0; P.B[1 * PL + c0] = n1; P.B[2 * PL + c0] = n2;
     if (P.last && P.Bavg) {
@@ -155,10 +160,10 @@ __global__ void maxwell_B_kernel(MaxParams P) {
 int launch_maxwell(vlasov_ctx* c, double dt, int nsub, double* E, double* B, const double* J, double* Bavg) {
     MaxParams P;
     P.E = E; P.B = B; P.J = J; P.Bavg = Bavg;
-    P.nx = c->G.nx; P.nyg = c->G.nyg; P.wall = c->G.wall;
-    P.dx = c->G.dx; P.dy = c->G.dy; P.c = c->c; P.mu0 = c->mu0;
+    P.nx = c->G.nx; P.nyg = c->G.nyg; P.nz = c->G.nz; P.wall = c->G.wall;
+    P.dx = c->G.dx; P.dy = c->G.dy; P.dz = c->G.dz; P.c = c->c; P.mu0 = c->mu0;
     P.ddt = dt / nsub;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     const int blocks = (ncell + 127) / 128;
     for (int sub = 0; sub < nsub; ++sub) {
         P.last = sub == nsub - 1;

@@ -144,41 +144,44 @@ struct CurParams {
     const double* __restrict__ mom;   // [ns][11][ncell]
     double* __restrict__ J;
     double q[MAX_SPECIES];
-    int ns, nx, nyg, fields_yee, wall;
+    int ns, nx, nyg, nz, fields_yee, wall;
 };
 
-__device__ __forceinline__ double jc_at(const CurParams& P, int d, int j, int i) {
-    const long PL = (long)P.nx * P.nyg;
+__device__ __forceinline__ double jc_at(const CurParams& P, int d, int k, int j, int i) {
+    const long PL = (long)P.nx * P.nyg * P.nz;
     double r = 0.0;
-    for (int s = 0; s < P.ns; ++s) r += P.q[s] * P.mom[((long)s * 11 + 1 + d) * PL + (long)j * P.nx + i];
+    for (int s = 0; s < P.ns; ++s) r += P.q[s] * P.mom[((long)s * 11 + 1 + d) * PL + ((long)k * P.nyg + j) * P.nx + i];
     return r;
 }
 
+// J at the E positions of the Yee grid (R17 / R24): Jx(i+1/2,j,k) averages the cell-centre currents over (j-1,j) x
+// (k-1,k), Jy(i,j+1/2,k) over (i-1,i) x (k-1,k), Jz(i,j,k+1/2) over (i-1,i) x (j-1,j).  With nz = 1 the z neighbour
+// is the cell itself and the sums are the 2D ones bit for bit.
 __global__ void current_kernel(CurParams P) {
     const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     if (cell >= ncell) return;
-    const int j = cell / P.nx, i = cell % P.nx;
+    const int i = cell % P.nx, j = (cell / P.nx) % P.nyg, k = cell / (P.nx * P.nyg);
     const long PL = ncell;
     if (!P.fields_yee) {
-        for (int d = 0; d < 3; ++d) P.J[d * PL + cell] = jc_at(P, d, j, i);
+        for (int d = 0; d < 3; ++d) P.J[d * PL + cell] = jc_at(P, d, k, j, i);
         return;
     }
-    const int im = (i + P.nx - 1) % P.nx;
+    const int im = (i + P.nx - 1) % P.nx, km = (k + P.nz - 1) % P.nz;
     int jm = j - 1;
     bool onwall = false;
     if (jm < 0) { jm = P.nyg - 1; onwall = P.wall != 0; }
-    P.J[0 * PL + cell] = onwall ? 0.0 : 0.5 * (jc_at(P, 0, jm, i) + jc_at(P, 0, j, i));
-    P.J[1 * PL + cell] = 0.5 * (jc_at(P, 1, j, im) + jc_at(P, 1, j, i));
-    P.J[2 * PL + cell] = onwall ? 0.0 : 0.25 * (jc_at(P, 2, jm, im) + jc_at(P, 2, jm, i) + jc_at(P, 2, j, im) + jc_at(P, 2, j, i));
+    P.J[0 * PL + cell] = onwall ? 0.0 : 0.25 * ((jc_at(P, 0, km, jm, i) + jc_at(P, 0, km, j, i)) + (jc_at(P, 0, k, jm, i) + jc_at(P, 0, k, j, i)));
+    P.J[1 * PL + cell] = 0.25 * ((jc_at(P, 1, km, j, im) + jc_at(P, 1, km, j, i)) + (jc_at(P, 1, k, j, im) + jc_at(P, 1, k, j, i)));
+    P.J[2 * PL + cell] = onwall ? 0.0 : 0.25 * (jc_at(P, 2, k, jm, im) + jc_at(P, 2, k, jm, i) + jc_at(P, 2, k, j, im) + jc_at(P, 2, k, j, i));
 }
 
 int launch_current(vlasov_ctx* c, double* J) {
     CurParams P;
     P.mom = c->mom; P.J = J;
-    P.ns = c->ns; P.nx = c->G.nx; P.nyg = c->G.nyg; P.fields_yee = c->G.fields_yee; P.wall = c->G.wall;
+    P.ns = c->ns; P.nx = c->G.nx; P.nyg = c->G.nyg; P.nz = c->G.nz; P.fields_yee = c->G.fields_yee; P.wall = c->G.wall;
     for (int s = 0; s < c->ns; ++s) P.q[s] = c->sp[s].q;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     {
         Launch L(c, K_CURRENT);
         current_kernel<<<(ncell + 127) / 128, 128, 0, c->stream>>>(P);

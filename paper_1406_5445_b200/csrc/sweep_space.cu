@@ -19,7 +19,8 @@ struct SpaceParams {
     int n_line;        // cells along the line that are UPDATED (x: nx, y: ny)
     int nx, ny, g, nyg;
     int nv1, nv2;      // nv[1], nv[2]
-    int axis;          // 0: x sweep, 1: y sweep
+    int axis;          // 0: x sweep, 1: y sweep, 2: z sweep (3D3V, periodic)
+    long slab;         // doubles per z slab (y sweep: blockIdx.z picks the slab)
     double vmin, dv;   // velocity direction that sets sigma
     double dts, dxx;
     double finf;
@@ -53,7 +54,7 @@ __device__ __forceinline__ Pack<VEC> fetch(const SpaceParams& P, const double* b
     const int N = P.n_line;
     if (r >= 0 && r < N) return ld<VEC>(base + (long)r * P.line_stride);
     long off = 0;
-    if (P.axis == 0) {                      // x: periodic
+    if (P.axis != 1) {                      // x, z: periodic
         while (r < 0) r += N;
         while (r >= N) r -= N;
         return ld<VEC>(base + (long)r * P.line_stride);
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     const long v = chunk * VEC;
     const int ivx = (int)(v / ((long)P.nv1 * P.nv2));
     const int ivy = (int)((v / P.nv2) % P.nv1);
-    const int other = P.row0 + blockIdx.y;  // x sweep: ghost-inclusive row; y sweep: ix
+    const int other = P.row0 + blockIdx.y;  // x sweep: row (of all slabs); y sweep: ix; z sweep: spatial cell of a slab
     const double* base;
     double* obase;
     long mir = 0;
@@ -92,16 +93,21 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
         base = P.src + ((long)other * P.nx) * P.S + v;
         obase = P.dst + ((long)other * P.nx) * P.S + v;
         vc = P.vmin + (ivx + 0.5) * P.dv;
+    } else if (P.axis == 2) {
+        base = P.src + (long)other * P.S + v;
+        obase = P.dst + (long)other * P.S + v;
+        vc = P.vmin + ((int)(v % P.nv2) + 0.5) * P.dv;      // VEC = 1: one v_z cell per thread
     } else {
-        base = P.src + ((long)P.g * P.nx + other) * P.S + v;
-        obase = P.dst + ((long)P.g * P.nx + other) * P.S + v;
+        const long zo = (long)blockIdx.z * P.slab;
+        base = P.src + zo + ((long)P.g * P.nx + other) * P.S + v;
+        obase = P.dst + zo + ((long)P.g * P.nx + other) * P.S + v;
         mir = (long)(P.nv1 - 1 - 2 * ivy) * P.nv2;
         vc = P.vmin + (ivy + 0.5) * P.dv;
         // ghost rows are Dirichlet data (R16): carried over unchanged
         for (int r = 0; r < P.g; ++r) {
-            st<VEC>(P.dst + ((long)r * P.nx + other) * P.S + v, ld<VEC>(P.src + ((long)r * P.nx + other) * P.S + v));
+            st<VEC>(P.dst + zo + ((long)r * P.nx + other) * P.S + v, ld<VEC>(P.src + zo + ((long)r * P.nx + other) * P.S + v));
             long rr = P.g + P.ny + r;
-            st<VEC>(P.dst + (rr * P.nx + other) * P.S + v, ld<VEC>(P.src + (rr * P.nx + other) * P.S + v));
+            st<VEC>(P.dst + zo + (rr * P.nx + other) * P.S + v, ld<VEC>(P.src + zo + (rr * P.nx + other) * P.S + v));
         }
     }
     const int N = P.n_line;
@@ -109,7 +115,7 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     const int u = sigma >= 0.0 ? 1 : -1;
     int n; double b;
     split_shift(fabs(sigma), n, b);
-    const bool periodic = P.axis == 0 || (P.bc_lo == VLASOV_BC_PERIODIC && P.bc_hi == VLASOV_BC_PERIODIC);
+    const bool periodic = P.axis != 1 || (P.bc_lo == VLASOV_BC_PERIODIC && P.bc_hi == VLASOV_BC_PERIODIC);
     if (periodic) n %= N;
     bool bad = false;
 
@@ -159,20 +165,25 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
     P.axis = axis;
     P.nx = G.nx; P.ny = G.ny; P.g = G.g; P.nyg = G.nyg;
     P.nv1 = s.nv[1]; P.nv2 = s.nv[2];
-    P.line_stride = axis == 0 ? s.nvtot : (long)G.nx * s.nvtot;
-    P.n_line = axis == 0 ? G.nx : G.ny;
+    P.slab = (long)G.nyg * G.nx * s.nvtot;
+    P.line_stride = axis == 0 ? s.nvtot : axis == 1 ? (long)G.nx * s.nvtot : P.slab;
+    P.n_line = axis == 0 ? G.nx : axis == 1 ? G.ny : G.nz;
     P.vmin = s.vmin[axis]; P.dv = s.dv[axis];
-    P.dts = dts; P.dxx = axis == 0 ? G.dx : G.dy;
+    P.dts = dts; P.dxx = axis == 0 ? G.dx : axis == 1 ? G.dy : G.dz;
     P.finf = s.f_inf; P.limiter = G.limiter;
     P.bc_lo = G.bc_lo; P.bc_hi = G.bc_hi;
     P.err = c->errflag;
     P.row0 = axis == 0 ? row0 : 0;
-    if (nrows < 0) nrows = G.nyg;
+    if (nrows < 0) nrows = G.nrows;              // x sweep: the rows of every z slab
     if (nrows == 0) return VLASOV_OK;
     const int threads = 128;
-    const long chunks = s.nvtot / 2;
-    dim3 grid((unsigned)((chunks + threads - 1) / threads), (unsigned)(axis == 0 ? nrows : G.nx));
-    {
+    if (axis == 2) {                             // sigma depends on i_vz: one v_z cell per thread
+        dim3 grid((unsigned)((s.nvtot + threads - 1) / threads), (unsigned)(G.nyg * G.nx));
+        Launch L(c, K_SWEEP_Z);
+        sweep_space_kernel<1, 4><<<grid, threads, 0, c->stream>>>(P);
+    } else {
+        const long chunks = s.nvtot / 2;
+        dim3 grid((unsigned)((chunks + threads - 1) / threads), (unsigned)(axis == 0 ? nrows : G.nx), (unsigned)(axis == 0 ? 1 : G.nz));
         Launch L(c, axis == 0 ? K_SWEEP_X : K_SWEEP_Y);
         sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
     }
@@ -187,6 +198,9 @@ int launch_sweep_x_rows(vlasov_ctx* c, const Species& s, const double* src, doub
 }
 int launch_sweep_y(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts) {
     return launch_space(c, s, src, dst, dts, 1);
+}
+int launch_sweep_z(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts) {
+    return launch_space(c, s, src, dst, dts, 2);
 }
 
 }  // namespace vl

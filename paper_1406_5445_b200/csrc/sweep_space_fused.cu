@@ -30,6 +30,7 @@ struct XYParams {
     long S;            // doubles per spatial cell
     long row_stride;   // nx * S
     int nx, ny, g;
+    int nyg;           // rows of a z slab (3D3V: blockIdx.y is the slab)
     int nv1, nv2;
     int C;             // contiguous velocity cells per CTA
     int PC;            // cells per bulk copy (a piece of one v_z row, or the whole chunk)
@@ -214,7 +215,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
             for (int p = 0; p < npp; ++p) {
                 long vp = v0 + (long)p * PC;
                 if (m) vp += (long)(nv1 - 1 - 2 * (int)((vp / nv2) % nv1)) * nv2;
-                tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes, &tmap, (int)vp, ar * nx, bar);
+                tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes, &tmap, (int)vp, (ar + (int)blockIdx.y * P.nyg) * nx, bar);
             }
         }
     };
@@ -243,7 +244,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
         const unsigned sraw = raw0 + stage * rowbytes;
         mbar_wait(bar0 + 8 * stage, phase);
         const int orow = r - orow_shift;
-        double* po = P.dst + (long)(P.g + orow) * row_stride + (long)ix0 * S + v;
+        double* po = P.dst + (long)(P.g + orow + (int)blockIdx.y * P.nyg) * row_stride + (long)ix0 * S + v;
         const bool store = orow >= 0 && orow < P.ny;
         const int nstage = stage == 0 ? XY_NS - 1 : stage - 1;      // stage of row r + NS - 1 = stage of row r - 1
         if (XFIRST) {
@@ -404,7 +405,7 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     XYParams P;
     P.src = src; P.dst = dst;
     P.S = s.nvtot; P.row_stride = (long)G.nx * s.nvtot;
-    P.nx = G.nx; P.ny = G.ny; P.g = G.g;
+    P.nx = G.nx; P.ny = G.ny; P.g = G.g; P.nyg = G.nyg;
     P.nv1 = s.nv[1]; P.nv2 = s.nv[2];
     P.vminx = s.vmin[0]; P.dvx = s.dv[0]; P.vminy = s.vmin[1]; P.dvy = s.dv[1];
     P.kx = dts / G.dx; P.ky = dts / G.dy;
@@ -417,8 +418,8 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     P.PC = C < s.nv[2] ? C : s.nv[2];
     const size_t smem = xy_smem_bytes(G, s, C, xfirst);
     CUtensorMap tm;
-    if (!make_tensor_map_2d(&tm, src, s.nvtot, (long)G.nyg * G.nx, P.PC, G.nx)) return VLASOV_ECUDA;
-    dim3 grid((unsigned)(s.nvtot / C));
+    if (!make_tensor_map_2d(&tm, src, s.nvtot, (long)G.nrows * G.nx, P.PC, G.nx)) return VLASOV_ECUDA;
+    dim3 grid((unsigned)(s.nvtot / C), (unsigned)G.nz);
     const int threads = nblk * C;
     const int lim = G.limiter ? 1 : 0;
     {

@@ -30,7 +30,7 @@ struct TableParams {
     const double* __restrict__ E;
     const double* __restrict__ B;
     double* __restrict__ table;
-    int nx, nyg, fields_yee, wall;
+    int nx, nyg, nz, fields_yee, wall;
     double qm_half_dt;        // (q/m)(dt/2), eqs. (26), (28)
     double vmin[3], dv[3];
     double finf;
@@ -39,27 +39,28 @@ struct TableParams {
 
 __global__ void lorentz_table_kernel(TableParams P) {
     const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     if (cell >= ncell) return;
-    const int j = cell / P.nx, ix = cell % P.nx;
+    const int ix = cell % P.nx, j = (cell / P.nx) % P.nyg, k = cell / (P.nx * P.nyg);
     const long PL = (long)ncell;
     double Ec[3], Bc[3];
     if (!P.fields_yee) {
         for (int d = 0; d < 3; ++d) { Ec[d] = P.E[d * PL + cell]; Bc[d] = P.B[d * PL + cell]; }
     } else {
-        // cell (i,j) spans [i dx,(i+1)dx] x [j dy,(j+1)dy]; Ex(i+1/2,j) Ey(i,j+1/2) Ez(i,j)
-        // Bx(i,j+1/2) By(i+1/2,j) Bz(i+1/2,j+1/2): linear interpolation to the centre
-        int ip = (ix + 1) % P.nx;
+        // cell (i,j,k) spans [i dx,(i+1)dx] x [j dy,(j+1)dy] x [k dz,(k+1)dz]; Ex(i+1/2,j,k) Ey(i,j+1/2,k) Ez(i,j,k+1/2)
+        // Bx(i,j+1/2,k+1/2) By(i+1/2,j,k+1/2) Bz(i+1/2,j+1/2,k) (R17 / R24): linear interpolation to the centre.
+        // With nz = 1 the z neighbour is the cell itself and the sums below are the 2D ones bit for bit.
+        const int ip = (ix + 1) % P.nx, kp = (k + 1) % P.nz;
         int jp = j + 1;
         double up = 1.0;
         if (jp >= P.nyg) { jp = 0; if (P.wall) up = 0.0; }
-        auto at = [&](const double* A, int d, int jj, int ii) { return A[d * PL + (long)jj * P.nx + ii]; };
-        Ec[0] = 0.5 * (at(P.E, 0, j, ix) + up * at(P.E, 0, jp, ix));
-        Ec[1] = 0.5 * (at(P.E, 1, j, ix) + at(P.E, 1, j, ip));
-        Ec[2] = 0.25 * (at(P.E, 2, j, ix) + at(P.E, 2, j, ip) + up * at(P.E, 2, jp, ix) + up * at(P.E, 2, jp, ip));
-        Bc[0] = 0.5 * (at(P.B, 0, j, ix) + at(P.B, 0, j, ip));
-        Bc[1] = 0.5 * (at(P.B, 1, j, ix) + up * at(P.B, 1, jp, ix));
-        Bc[2] = at(P.B, 2, j, ix);
+        auto at = [&](const double* A, int d, int kk, int jj, int ii) { return A[d * PL + ((long)kk * P.nyg + jj) * P.nx + ii]; };
+        Ec[0] = 0.25 * ((at(P.E, 0, k, j, ix) + up * at(P.E, 0, k, jp, ix)) + (at(P.E, 0, kp, j, ix) + up * at(P.E, 0, kp, jp, ix)));
+        Ec[1] = 0.25 * ((at(P.E, 1, k, j, ix) + at(P.E, 1, k, j, ip)) + (at(P.E, 1, kp, j, ix) + at(P.E, 1, kp, j, ip)));
+        Ec[2] = 0.25 * (at(P.E, 2, k, j, ix) + at(P.E, 2, k, j, ip) + up * at(P.E, 2, k, jp, ix) + up * at(P.E, 2, k, jp, ip));
+        Bc[0] = 0.5 * (at(P.B, 0, k, j, ix) + at(P.B, 0, k, j, ip));
+        Bc[1] = 0.5 * (at(P.B, 1, k, j, ix) + up * at(P.B, 1, k, jp, ix));
+        Bc[2] = 0.5 * (at(P.B, 2, k, j, ix) + at(P.B, 2, kp, j, ix));
     }
     // eq. (28): t = (q/m)(dt/2) B, s = 2t/(1+t^2); eq. (26): h = (q/m)(dt/2) E
     const double tx = P.qm_half_dt * Bc[0], ty = P.qm_half_dt * Bc[1], tz = P.qm_half_dt * Bc[2];
@@ -110,12 +111,12 @@ __global__ void lorentz_table_kernel(TableParams P) {
 int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const double* B, double dt) {
     TableParams P;
     P.E = E; P.B = B; P.table = c->table;
-    P.nx = c->G.nx; P.nyg = c->G.nyg; P.fields_yee = c->G.fields_yee; P.wall = c->G.wall;
+    P.nx = c->G.nx; P.nyg = c->G.nyg; P.nz = c->G.nz; P.fields_yee = c->G.fields_yee; P.wall = c->G.wall;
     P.qm_half_dt = (s.q / s.m) * (dt / 2.0);
     for (int d = 0; d < 3; ++d) { P.vmin[d] = s.vmin[d]; P.dv[d] = s.dv[d]; }
     P.finf = s.f_inf;
     P.err = c->errflag;
-    const int ncell = P.nx * P.nyg;
+    const int ncell = P.nx * P.nyg * P.nz;
     {
         Launch L(c, K_TABLE);
         lorentz_table_kernel<<<(ncell + 127) / 128, 128, 0, c->stream>>>(P);
@@ -888,10 +889,10 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 16) k = lim ? vsweep_x_kernel<1, 16> : vsweep_x_kernel<0, 16>;
         if (spec == 32) k = lim ? vsweep_x_kernel<1, 32> : vsweep_x_kernel<0, 32>;
         const int tspec = (cn == 16 || cn == 24 || cn == 32 || cn == 40 || cn == 48) ? cn : 0;
-        if (tspec && !ghost && (long)c->G.nyg * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
+        if (tspec && !ghost && (long)c->G.nrows * c->G.nx * s.nv[0] < 2147483647L) {      // TMA coordinates are 32-bit
             // prefetching variant: one CUtensorMap over f as a matrix [cells * nv0][nv1 * nv2]; its own tile shape
             CUtensorMap tm;
-            if (!make_tensor_map_2d(&tm, src, plane, (long)c->G.nyg * c->G.nx * s.nv[0], 128, tspec)) return VLASOV_ECUDA;
+            if (!make_tensor_map_2d(&tm, src, plane, (long)c->G.nrows * c->G.nx * s.nv[0], 128, tspec)) return VLASOV_ECUDA;
             P.ct = 128; P.nseg = tspec / 8;
             P.ntile = (plane + 127) / 128;
             P.ntot = P.ntile * ncell;
@@ -934,10 +935,10 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 32) k = lim ? vsweep_yz_kernel<1, 32> : vsweep_yz_kernel<0, 32>;
         if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
         if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
-        if (spec && spec != 48 && (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1] < 2147483647L) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
+        if (spec && spec != 48 && (long)c->G.nrows * c->G.nx * s.nv[0] * s.nv[1] < 2147483647L) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
             // TMA-staged variant: f as a matrix [cells * nv0 * nv1][nv2], one box {nv2, nv1} per plane
             CUtensorMap tm;
-            if (!make_tensor_map_2d(&tm, f, s.nv[2], (long)c->G.nyg * c->G.nx * s.nv[0] * s.nv[1], s.nv[2], s.nv[1])) return VLASOV_ECUDA;
+            if (!make_tensor_map_2d(&tm, f, s.nv[2], (long)c->G.nrows * c->G.nx * s.nv[0] * s.nv[1], s.nv[2], s.nv[1])) return VLASOV_ECUDA;
             void (*kt)(CUtensorMap, VParams) = lim ? vsweep_yz_tma_kernel<1, 32> : vsweep_yz_tma_kernel<0, 32>;
             if (spec == 16) kt = lim ? vsweep_yz_tma_kernel<1, 16> : vsweep_yz_tma_kernel<0, 16>;
             if (spec == 24) kt = lim ? vsweep_yz_tma_kernel<1, 24> : vsweep_yz_tma_kernel<0, 24>;

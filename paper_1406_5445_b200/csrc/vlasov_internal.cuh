@@ -28,7 +28,8 @@ struct Species {
 
 struct Geom {
     int nx, ny, g, nyg;
-    double dx, dy;
+    int nz, nrows;     // 3D3V: slabs along z (1 = the 2D path); nrows = nz * nyg = all rows of an array
+    double dx, dy, dz;
     int bc_lo, bc_hi;
     int limiter, fields_yee, wall;
 };
@@ -73,7 +74,7 @@ namespace vl {
 
 enum Kind { K_SWEEP_X = 0, K_SWEEP_Y, K_TABLE, K_VSWEEP_X, K_VSWEEP_YZ, K_MOMENTS, K_GHOST_TABLE, K_CURRENT,
             K_MAXWELL, K_SWEEP_XY, K_SWEEP_YX, K_GHOST_VSWEEP_X, K_GHOST_VSWEEP_YZ, K_GHOST_MOMENTS, K_GHOST_SWEEP_X,
-            K_COUNT };
+            K_SWEEP_Z, K_COUNT };
 static_assert((int)K_COUNT == (int)VLASOV_KIND_COUNT, "kinds of vlasov.h");
 
 // Counts a launch and, when timing is on, brackets it with an event pair on the context's stream.
@@ -102,6 +103,7 @@ struct Launch {
 // spatial half sweeps, out of place src -> dst (a1, a2, a7, a8 of DESIGN.md)
 int launch_sweep_x(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);
 int launch_sweep_y(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);
+int launch_sweep_z(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts);   // 3D3V, periodic
 // x sweep of rows [row0, row0+nrows) only (ghost rows beside a fused stage)
 int launch_sweep_x_rows(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int row0, int nrows);
 // fused spatial stage (sweep_space_fused.cu): x then y (xfirst) or y then x, interior rows, src -> dst

@@ -59,6 +59,8 @@ class Workload:
     seed: int = 1
     kind: str = "gem"     # "landau" | "gem" | "band"
     y_centre_offset: float = 0.0
+    nz: int = 1           # 3D3V (NEXT-4): cells along z, periodic
+    lz: float = 1.0
 
     @property
     def ny_g(self):
