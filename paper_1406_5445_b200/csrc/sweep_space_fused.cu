@@ -16,8 +16,8 @@
 // Rows -2, -1 and ny, ny+1 are the boundary rows of the y sweep (R16, R19): periodic wrap, the wall
 // image f(y_w + eta, vy) = f(y_w - eta, -vy), or FLUID ghost rows; they are loaded like any row.
 #include <mutex>
-#include <set>
-#include <tuple>
+#include <map>
+#include <utility>
 #include <type_traits>
 #include "vlasov_internal.cuh"
 #include "tma.cuh"
@@ -330,19 +330,20 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
     }
 }
 
-// The opt-in to more than 48 KiB of dynamic shared memory is a per-device function attribute: set once per
-// (device, kernel, size), not on every launch.
+// The opt-in to more than 48 KiB of dynamic shared memory is a per-device function attribute and a MAXIMUM: it is raised
+// when a launch needs more than any launch of that kernel on that device before it, never lowered.
 template <class K>
 static void ensure_smem_attr(K kernel, size_t smem) {
     static std::mutex mu;
-    static std::set<std::tuple<int, const void*, size_t>> done;
+    static std::map<std::pair<int, const void*>, size_t> granted;
     int dev = 0;
     cudaGetDevice(&dev);
-    const auto key = std::make_tuple(dev, (const void*)kernel, smem);
+    const auto key = std::make_pair(dev, (const void*)kernel);
     std::lock_guard<std::mutex> lock(mu);
-    if (done.count(key)) return;
+    auto it = granted.find(key);
+    if (it != granted.end() && it->second >= smem) return;
     cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    done.insert(key);
+    granted[key] = smem;
 }
 
 template <int XB, int LIM, int SP, int NV = 32, int KC = xy_default_chunk(SP)>
