@@ -33,7 +33,7 @@ UNIT = "cell-updates/s"
 
 # Algorithmic HBM bytes per phase-space cell and launch of each f-sized kernel:
 # a sweep reads and writes every cell once (8 + 8 B); the moments pass reads it once.
-BYTES_PER_CELL = {"sweep_x": 16.0, "sweep_y": 16.0, "sweep_xy": 16.0, "sweep_yx": 16.0, "vsweep_x": 16.0, "vsweep_yz": 16.0,
+BYTES_PER_CELL = {"sweep_x": 16.0, "sweep_y": 16.0, "sweep_z": 16.0, "sweep_xy": 16.0, "sweep_yx": 16.0, "vsweep_x": 16.0, "vsweep_yz": 16.0,
                   "vsweep_xyz": 16.0, "moments": 8.0}
 
 
@@ -44,6 +44,8 @@ def make_workload(name):
         return inputs.gem_workload(nx=64, ny=32, nv=32, steps=50, name="gem_64x32x32^3_x2species")
     if name == "band":
         return inputs.band_workload()
+    if name == "gem3d":
+        return inputs.gem3d_workload()
     if name.startswith("nv"):
         nv = int(name[2:])
         return inputs.gem_workload(nx=64, ny=64, nv=nv, steps=10, name=f"gem_64x64x{nv}^3_x2species")
@@ -212,6 +214,12 @@ def whole_job_value(cells_per_replica, steps, ms, world):
 def upload_f(w, s, torch, device):
     """Seeded f of species s, generated row by row on the host and copied to the device."""
     sp = w.species[s]
+    if getattr(w, "nz", 1) > 1:          # 3D3V: slab by slab
+        f = torch.empty((w.nz, w.ny_g, w.nx) + tuple(sp.nv), dtype=torch.float64, device=device)
+        for k in range(w.nz):
+            f[k].copy_(torch.from_numpy(inputs.gem3d_f(w, s, k)))
+        sp.f_inf = inputs.gem_f_inf(w, s)
+        return f
     f = torch.empty((w.ny_g, w.nx) + tuple(sp.nv), dtype=torch.float64, device=device)
     for r in range(w.ny_g):
         f[r].copy_(torch.from_numpy(inputs.gem_f(w, s, rows=[r])[0]))
@@ -240,7 +248,8 @@ def gpu_arm(args):
     w = make_workload(args.workload)
     ns = len(w.species)
     fs = [upload_f(w, s, torch, device) for s in range(ns)]
-    E0, B0 = inputs.gem_fields(w)
+    nz = getattr(w, "nz", 1)
+    E0, B0 = inputs.gem3d_fields(w) if nz > 1 else inputs.gem_fields(w)
     stream = torch.cuda.current_stream()
     order = binding.ORDER_VXV if args.order == "vxv" else binding.ORDER_XVX
     ctx = binding.context_for(w, fs, order=order)
@@ -340,7 +349,7 @@ def gpu_arm(args):
     ctx.vlasov_check()
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms = float(np.median(rep_ms))
-    cells = w.interior_cells
+    cells = w.interior_cells * nz
     value = whole_job_value(cells, args.steps, ms, world)
 
     # ---- the same number of steps again with an event pair around every launch: the per-kernel table ----
@@ -356,10 +365,10 @@ def gpu_arm(args):
     ctx.vlasov_timing_enable(False)
 
     # ---- end-to-end leg: HOST buffers through the C ABI (vlasov_cycle_host) -----------------
-    ncell = w.ny_g * w.nx
+    ncell = w.ny_g * w.nx * nz
     Eh = torch.from_numpy(E0.copy()).pin_memory()
     Bh = torch.from_numpy(B0.copy()).pin_memory()
-    Mh = torch.empty((ns, 10, w.ny_g, w.nx), dtype=torch.float64).pin_memory()
+    Mh = torch.empty((ns, 10, nz * w.ny_g, w.nx), dtype=torch.float64).pin_memory()
     Eh.copy_(Ed.cpu()); Bh.copy_(Bd.cpu())
     e2e_steps = max(1, min(args.steps, 10))
     set_fluid()
@@ -387,7 +396,7 @@ def gpu_arm(args):
 
     # ---- roofline of the dominant kernel (CUDA-event pairs around every launch, timed region) ----
     peak, peak_src = peaks()
-    cells_all = sum(w.ny_g * w.nx * s.ncell_v for s in w.species) / ns      # ghost-inclusive, per species launch
+    cells_all = sum(nz * w.ny_g * w.nx * s.ncell_v for s in w.species) / ns  # ghost-inclusive, per species launch
     cells_int = cells / ns                                                     # interior rows only
     kinds = {}
     tot_ms = sum(v[0] for v in per_kind.values())
@@ -445,7 +454,7 @@ def gpu_arm(args):
 
     # ---- the oracle timed beside it (reported baseline only) --------------------------------
     cpu = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and nz == 1:        # (the oracle leg samples 2D cuts; the 3D workload is timed without it)
         v, _, cores, sample, _ = oracle_leg(make_workload(args.workload), steps=50, warmup=1, budget_s=args.cpu_budget)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle", "sample": sample}
 
@@ -456,7 +465,7 @@ def gpu_arm(args):
                    "repetitions": len(rep_ms), "ms_per_step_each": [m / args.steps for m in rep_ms],
                    "ms_per_step_with_per_launch_events": ms_instr / args.steps},
         "dtype": "f64", "data": "synthetic (seeded GEM Harris-sheet profiles + hash noise, DESIGN.md 'Input recipe')",
-        "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nghost_y": w.nghost_y,
+        "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": nz, "nghost_y": w.nghost_y,
                    "nv": list(w.species[0].nv), "species": ns, "dt": w.dt, "maxwell_nsub": w.nsub,
                    "interior_cells_per_step": cells,
                    "fluid": (args.fluid if fluid is not None else None),

@@ -13,7 +13,8 @@
 //
 // Pins (tests/test_oracle_*.py): T1..T17 of DESIGN.md, the VXV pins (orc_step with order = 1: T10/T11/T5/T16 under
 // that order, Landau rate under VXV), the PEC-row pins of orc_field_at_cell and orc_current, and -- for the cycle
-// composed from these functions in oracle.py -- C1, C2.  Every function here is pinned.  Readings the paper leaves
+// composed from these functions in oracle.py -- C1, C2; the 3D3V functions at the end of this file: D1..D6
+// (tests/test_oracle_3d.py).  Every function here is pinned.  Readings the paper leaves
 // open and for which no outside fact exists are DECLARED DEFINITIONS: limiter under compressive
 // velocity shifts (R6/R15d), zeroth-order ghost extrapolation (R15a), isotropic target temperature (R15c), ghost-row
 // Dirichlet reuse (R16), the choice of Yee positions (R17).

@@ -300,3 +300,32 @@ def band_fluid_block(w: Workload, nyf: int, side: int):
         U[s, 3] = sp.m * n * uz
         U[s, 4] = 1.5 * n * T + 0.5 * sp.m * n * uz ** 2
     return U, E, B
+
+
+# ------------------------------------------------------------------------------------------------
+# 3D3V (NEXT-4): the Harris sheet extruded along z (uniform in z up to the noise), z periodic
+# ------------------------------------------------------------------------------------------------
+def gem3d_workload(nx=32, ny=32, nz=8, nv=32, steps=10, dt=0.005, seed=1, lx=25.6, ly=12.8, lz=6.4, name=None) -> Workload:
+    w = gem_workload(nx=nx, ny=ny, nv=nv, steps=steps, dt=dt, seed=seed, lx=lx, ly=ly,
+                     name=name or f"gem3d_{nx}x{ny}x{nz}x{nv}^3_x2species")
+    w.nz, w.lz = nz, lz
+    w.nsub = _nsub_for(w.c, dt / 2, min(w.dx, lz / nz), w.dy)
+    w.kind = "gem3d"
+    return w
+
+
+def gem3d_f(w: Workload, s: int, k: int) -> np.ndarray:
+    """Slab k of f_s [ny, nx, nvx, nvy, nvz]: the 2D Harris state with its own noise stream."""
+    seed = w.seed
+    w.seed = seed + 7919 * (k + 1)
+    try:
+        return gem_f(w, s)
+    finally:
+        w.seed = seed
+
+
+def gem3d_fields(w: Workload):
+    """[3, nz, ny, nx]: the 2D fields at every z (they do not depend on z)."""
+    E, B = gem_fields(w)
+    rep = lambda A: np.ascontiguousarray(np.broadcast_to(A[:, None], (3, w.nz) + A.shape[1:]))
+    return rep(E), rep(B)
