@@ -656,14 +656,18 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
 // a CTA = one work item (an 8-cell segment of one line) per thread, rounded up to whole warps.
 __host__ __device__ constexpr int yz_tma_planes(int cn) { return 2048 / (cn * cn) > 0 ? 2048 / (cn * cn) : 1; }
 __host__ __device__ constexpr int yz_tma_threads(int cn) { return (yz_tma_planes(cn) * cn * ((cn + 7) / 8) + 31) / 32 * 32; }
-static_assert(yz_tma_threads(32) == 256 && yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(40) == 224, "");
+static_assert(yz_tma_threads(32) == 256 && yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(40) == 224 &&
+              yz_tma_threads(48) == 288, "");
+// resident CTAs per SM the kernel is compiled for: 3 (80 registers at 256 threads); one 48x48 plane has 288 work items
+// (9 warps) and 69 KB of shared memory: 2 CTAs per SM
+__host__ __device__ constexpr int yz_tma_minb(int cn) { return cn == 48 ? 2 : VL_YZ_MINB; }
 
 // MOM = 1 (VXV order): the 10 raw velocity moments, eqs. (2)-(4), of the final f are
 // reduced in this kernel.  A CTA then takes WHOLE spatial cells (all tiles of a cell one after the other), sums its
 // cells while it stores them, and writes the moments of the cell itself: no partial sums in global memory, no
 // atomics, a fixed summation order.  For planes where a thread keeps its i_vz over a tile (16x16, 32x32).
 template <int LIM, int CN, int MOM = 0>
-__global__ void __launch_bounds__(yz_tma_threads(CN), VL_YZ_MINB) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
+__global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
     extern __shared__ __align__(128) double sm[];
     constexpr int N1 = CN, N2 = CN, plane = CN * CN;
     constexpr int ct = yz_tma_planes(CN);
@@ -935,7 +939,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
         if (spec == 32) k = lim ? vsweep_yz_kernel<1, 32> : vsweep_yz_kernel<0, 32>;
         if (spec == 40) k = lim ? vsweep_yz_kernel<1, 40> : vsweep_yz_kernel<0, 40>;
         if (spec == 48) k = lim ? vsweep_yz_kernel<1, 48> : vsweep_yz_kernel<0, 48>;
-        if (spec && spec != 48 && (long)c->G.nrows * c->G.nx * s.nv[0] * s.nv[1] < 2147483647L) {                      // (48x48 planes measured faster on the plain kernel: 2 CTAs per SM either way)
+        if (spec && (long)c->G.nrows * c->G.nx * s.nv[0] * s.nv[1] < 2147483647L) {
             // TMA-staged variant: f as a matrix [cells * nv0 * nv1][nv2], one box {nv2, nv1} per plane
             CUtensorMap tm;
             if (!make_tensor_map_2d(&tm, f, s.nv[2], (long)c->G.nrows * c->G.nx * s.nv[0] * s.nv[1], s.nv[2], s.nv[1])) return VLASOV_ECUDA;
@@ -943,6 +947,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (spec == 16) kt = lim ? vsweep_yz_tma_kernel<1, 16> : vsweep_yz_tma_kernel<0, 16>;
             if (spec == 24) kt = lim ? vsweep_yz_tma_kernel<1, 24> : vsweep_yz_tma_kernel<0, 24>;
             if (spec == 40) kt = lim ? vsweep_yz_tma_kernel<1, 40> : vsweep_yz_tma_kernel<0, 40>;
+            if (spec == 48) kt = lim ? vsweep_yz_tma_kernel<1, 48> : vsweep_yz_tma_kernel<0, 48>;
             const size_t srows = 8 + (size_t)pt * (s.nv[1] + 8);
             const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
             const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8 + 8 * 10 * 8;
@@ -955,7 +960,8 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
                 if (mom_done) *mom_done = true;
             }
             if (smem_t > V_SMEM_MAX) return VLASOV_EINVAL;
-            const int nt = spec == 16 ? yz_tma_threads(16) : spec == 24 ? yz_tma_threads(24) : spec == 40 ? yz_tma_threads(40) : yz_tma_threads(32);
+            const int nt = spec == 16 ? yz_tma_threads(16) : spec == 24 ? yz_tma_threads(24) : spec == 40 ? yz_tma_threads(40) :
+                           spec == 48 ? yz_tma_threads(48) : yz_tma_threads(32);
             const int grid = min(mom ? ncell : P.ntot, resident_ctas(kt, smem_t, nt));
             Launch L(c, K_VSWEEP_YZ);
             kt<<<grid, nt, smem_t, c->stream>>>(tm, P);
