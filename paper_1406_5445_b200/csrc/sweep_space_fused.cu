@@ -32,6 +32,7 @@ struct XYParams {
     int nx, ny, g;
     int nyg;           // rows of a z slab (3D3V: blockIdx.y is the slab)
     int nv1, nv2;
+    int nxb;           // x cells per TMA box (a box holds at most 256 rows: nx > 256 takes several boxes per row)
     int C;             // contiguous velocity cells per CTA
     int PC;            // cells per bulk copy (a piece of one v_z row, or the whole chunk)
     double vminx, dvx, vminy, dvy;
@@ -215,7 +216,10 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
             for (int p = 0; p < npp; ++p) {
                 long vp = v0 + (long)p * PC;
                 if (m) vp += (long)(nv1 - 1 - 2 * (int)((vp / nv2) % nv1)) * nv2;
-                tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes, &tmap, (int)vp, (ar + (int)blockIdx.y * P.nyg) * nx, bar);
+                const int nxb = SP ? SP : P.nxb;
+                for (int b = 0; b * nxb < nx; ++b)
+                    tma_g2s_2d(raw0 + stage * rowbytes + p * piecebytes + (unsigned)(b * nxb) * X8, &tmap, (int)vp,
+                               (ar + (int)blockIdx.y * P.nyg) * nx + b * nxb, bar);
             }
         }
     };
@@ -367,6 +371,12 @@ static size_t xy_smem_bytes(const Geom& G, const Species& s, int C, int xfirst) 
     return 128 + ((6 * (size_t)C * 8 + 127) & ~(size_t)127) + (xfirst ? XY_NS : XY_NS + 2) * row;
 }
 
+// x cells per TMA box: a box dimension is at most 256, so a row of nx > 256 cells arrives as nx / nxb equal boxes
+static int xy_box_rows(int nx) {
+    for (int k = 1; k <= 16; ++k) if (nx % k == 0 && nx / k <= 256) return nx / k;
+    return 0;
+}
+
 // Tile shape of the fused stage: XB x cells per thread, C contiguous velocity cells per CTA -- a power of two
 // that divides the block, made of whole v_z rows or a part of one, at least 16 bytes, at most 512 threads.
 static bool pick_xy_shape(const Geom& G, const Species& s, int& xb, int& C) {
@@ -378,7 +388,7 @@ static bool pick_xy_shape(const Geom& G, const Species& s, int& xb, int& C) {
     auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && nblk * cc <= VL_XY_MAXT; };
     while (C >= 2 && !ok(C)) C >>= 1;
     if (C < 2) return false;
-    if (G.nx > 256) return false;                  // TMA box limit
+    if (xy_box_rows(G.nx) == 0) return false;      // no equal split of a row into TMA boxes of at most 256 x cells
     return xy_smem_bytes(G, s, C, 0) <= 200 * 1024;
 }
 
@@ -419,7 +429,8 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
     P.PC = C < s.nv[2] ? C : s.nv[2];
     const size_t smem = xy_smem_bytes(G, s, C, xfirst);
     CUtensorMap tm;
-    if (!make_tensor_map_2d(&tm, src, s.nvtot, (long)G.nrows * G.nx, P.PC, G.nx)) return VLASOV_ECUDA;
+    P.nxb = xy_box_rows(G.nx);
+    if (!make_tensor_map_2d(&tm, src, s.nvtot, (long)G.nrows * G.nx, P.PC, P.nxb)) return VLASOV_ECUDA;
     dim3 grid((unsigned)(s.nvtot / C), (unsigned)G.nz);
     const int threads = nblk * C;
     const int lim = G.limiter ? 1 : 0;

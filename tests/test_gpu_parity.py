@@ -172,13 +172,14 @@ def test_spatial_half_steps(gpu, orc, bc, stages):
 @pytest.mark.parametrize("bc,g", [(inputs.BC_PERIODIC, 0), (inputs.BC_REFLECT, 0), (inputs.BC_FLUID, 2), (inputs.BC_FLUID, 3)])
 @pytest.mark.parametrize("nx,nv", [(13, (6, 8, 10)), (12, (4, 4, 8)), (16, (6, 8, 16)), (24, (3, 6, 32)),
                                    (64, (24, 24, 24)), (64, (32, 32, 32)), (128, (32, 32, 32)),
-                                   (64, (48, 48, 48)), (256, (40, 40, 40))])
+                                   (64, (48, 48, 48)), (256, (40, 40, 40)), (320, (4, 4, 8))])
 @pytest.mark.parametrize("stages", [1, 4])
 def test_fused_spatial_stage(gpu, orc, bc, g, nx, nv, stages):
     """a1+a2 / a7+a8 as ONE fused pass (all |sigma| < 1): x blocks of 1 and 4 cells, chunks of 2..32 velocity cells
     made of part of a v_z row / several rows, every y boundary kind; against the oracle and against the general
     one-direction kernels.  The shapes with nx = 64 / 128 / 256 are the compile-time-shape kernels of the benchmark
-    configs (32^3 with nx = 64 / 128; 24^3 and 48^3 of config 5 with nx = 64; 40^3 of config 4 with nx = 256)."""
+    configs (32^3 with nx = 64 / 128; 24^3 and 48^3 of config 5 with nx = 64; 40^3 of config 4 with nx = 256); nx = 320: a
+    row wider than one TMA box (256 rows) arrives as two boxes."""
     rng = np.random.default_rng(5)
     w = random_workload(rng, nx=nx, ny=7 if nx < 64 else 3, nv=nv, g=g, bc=bc)
     if nx >= 64:
