@@ -53,14 +53,19 @@ struct Weights {
     }
 };
 
-// Does the slope pair (dp, dm) of a cell with value f0 possibly need limiting?  High-word test of
-// vlasov_internal.cuh (conservative).  A comparison, not a difference: for f0 < 0 or f0 > f_inf (round-off leaves
-// -1e-17 behind) the high word of the bound is hugely negative and a difference would wrap around.
-__device__ __forceinline__ bool may_need(double f0, double dp, double dm, double finf) {
-    const int hb = min(__double2hiint(f0), __double2hiint(finf - f0)) + 0x00100000;
-    const int hp = __double2hiint(dp) & 0x7fffffff, hm = __double2hiint(dm) & 0x7fffffff;
-    return max(hp, hm) >= hb;
+// Can any of a batch of cells need its slopes limited?  High-word test of vlasov_internal.cuh, made once for the whole
+// batch from running integer minima / maxima (conservative; comparisons, not differences of high words: for f < 0 or
+// f > f_inf the high word of a bound is hugely negative):
+//     every |d| of the batch  <  min( 2 min f, 2 (f_inf - max f) )   ==>   every eps of the batch is 1.
+// hmin, hmax: signed min / max of the high words of the cells' values; dmax: max of the high words of |d| over every
+// difference the batch uses.  One fp64 subtraction per batch (f_inf minus an upper bound of max f) instead of one per
+// cell, 2 integer instructions per value instead of 6.
+__device__ __forceinline__ bool batch_may_need(int hmin, int hmax, int dmax, double finf) {
+    const double fmax_ub = __hiloint2double(hmax + 1, 0);          // > every value of the batch (f >= 0; else hmin < 0 decides)
+    const int hb = min(hmin, __double2hiint(finf - fmax_ub)) + 0x00100000;
+    return dmax >= hb;
 }
+__device__ __forceinline__ int hi_abs(double d) { return __double2hiint(d) & 0x7fffffff; }
 
 // N partial fluxes alpha [ f0 + c1 eps+ d+ + c2 eps- d- ] of the cells q[1..N] of a line piece q[0..N+1]
 // (q ordered in the direction of the flow, so eq. (47) is the same call on the reversed piece).
@@ -71,10 +76,13 @@ __device__ __forceinline__ void flux_line(const double (&q)[N + 2], const Weight
 #pragma unroll
     for (int i = 0; i <= N; ++i) d[i] = q[i + 1] - q[i];
     if (LIM) {
-        bool need = false;
+        int hmin = __double2hiint(q[1]), hmax = hmin, dmax = hi_abs(d[0]);
 #pragma unroll
-        for (int i = 0; i < N; ++i) need |= may_need(q[i + 1], d[i + 1], d[i], finf);
-        if (__any_sync(__activemask(), need)) {
+        for (int i = 1; i <= N; ++i) {
+            if (i < N) { hmin = min(hmin, __double2hiint(q[i + 1])); hmax = max(hmax, __double2hiint(q[i + 1])); }
+            dmax = max(dmax, hi_abs(d[i]));
+        }
+        if (__any_sync(__activemask(), batch_may_need(hmin, hmax, dmax, finf))) {
 #pragma unroll
             for (int i = 0; i < N; ++i) {
                 double sp, sm;
@@ -114,17 +122,20 @@ __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH],
 // NB steps of the y march at once (the owned cells of one x chunk): rows (r-2, r-1, r) = (ya, yb, gx) -> new average
 // h of row r-1 (sigma_y >= 0, eq. 46) or r-2 (sigma_y < 0, eq. 47 on the mirrored line).  One limiter vote for all
 // NB of them, so that the flux evaluations are independent instruction streams.
+// ydmax: max high word of |row r-1 - row r-2| over the batch, left by the previous row's call (where it was the upper
+// difference): the lower differences of this row need no second look.
 template <int NB, int LIM>
 __device__ __forceinline__ void y_batch(const double (&ya)[NB], const double (&yb)[NB], double (&yG)[NB],
-                                        const double (&gx)[NB], const Weights& Wy, double finf, double (&h)[NB]) {
+                                        const double (&gx)[NB], const Weights& Wy, double finf, double (&h)[NB], int& ydmax) {
     double dlo[NB], dhi[NB];
-    bool need = false;
+    int hmin = 0x7fffffff, hmax = (int)0x80000000, dup = 0;
 #pragma unroll
     for (int i = 0; i < NB; ++i) {
         dlo[i] = yb[i] - ya[i]; dhi[i] = gx[i] - yb[i];
-        if (LIM) need |= may_need(yb[i], dhi[i], dlo[i], finf);
+        if (LIM) { hmin = min(hmin, __double2hiint(yb[i])); hmax = max(hmax, __double2hiint(yb[i])); dup = max(dup, hi_abs(dhi[i])); }
     }
-    const bool slow = LIM && __any_sync(__activemask(), need);
+    const bool slow = LIM && __any_sync(__activemask(), batch_may_need(hmin, hmax, max(dup, ydmax), finf));
+    ydmax = dup;
 #pragma unroll
     for (int i = 0; i < NB; ++i) {
         double sp = Wy.pos ? dhi[i] : -dlo[i], sm = Wy.pos ? dlo[i] : -dhi[i];
@@ -238,6 +249,9 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
     for (int i = 0; i < XB; ++i) { A[i] = 0.0; B[i] = 0.0; yG[i] = 0.0; }
     const int orow_shift = ypos ? 1 : 2;
     constexpr int CH = XB < VL_XY_CH ? XB : VL_XY_CH;
+    int ydm[XB / CH];                              // limiter test of the y march: see y_batch
+#pragma unroll
+    for (int i = 0; i < XB / CH; ++i) ydm[i] = 0;
 
     // one row; PAR = parity of r + 2: rows (r-2, r-1) = (A, B) if PAR == 0 else (B, A); the new row replaces r-2
     auto row = [&](auto par, int r, int stage, unsigned phase) {
@@ -263,7 +277,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
                     double ya[CH], yb[CH], g[CH], h[CH];
 #pragma unroll
                     for (int i = 0; i < CH; ++i) { const int it = k * CH + i; ya[i] = PAR == 0 ? A[it] : B[it]; yb[i] = PAR == 0 ? B[it] : A[it]; g[i] = yG[it]; }
-                    y_batch<CH, LIM>(ya, yb, g, gx, Wy, finf, h);
+                    y_batch<CH, LIM>(ya, yb, g, gx, Wy, finf, h, ydm[k]);
 #pragma unroll
                     for (int i = 0; i < CH; ++i) {
                         const int it = k * CH + i;
@@ -276,7 +290,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
                     double ya[CH], yb[CH], g[CH], h[CH];
 #pragma unroll
                     for (int i = 0; i < CH; ++i) { const int it = XB - 1 - (k * CH + i); ya[i] = PAR == 0 ? A[it] : B[it]; yb[i] = PAR == 0 ? B[it] : A[it]; g[i] = yG[it]; }
-                    y_batch<CH, LIM>(ya, yb, g, gx, Wy, finf, h);
+                    y_batch<CH, LIM>(ya, yb, g, gx, Wy, finf, h, ydm[k]);
 #pragma unroll
                     for (int i = 0; i < CH; ++i) {
                         const int it = XB - 1 - (k * CH + i);
@@ -293,7 +307,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
                 double gx[XB], h[XB];
 #pragma unroll
                 for (int i = 0; i < XB; ++i) gx[i] = lds(sraw + own + i * X8);
-                if (PAR == 0) y_batch<XB, LIM>(A, B, yG, gx, Wy, finf, h); else y_batch<XB, LIM>(B, A, yG, gx, Wy, finf, h);
+                if (PAR == 0) y_batch<XB, LIM>(A, B, yG, gx, Wy, finf, h, ydm[0]); else y_batch<XB, LIM>(B, A, yG, gx, Wy, finf, h, ydm[0]);
 #pragma unroll
                 for (int i = 0; i < XB; ++i) {
                     if (PAR == 0) A[i] = gx[i]; else B[i] = gx[i];
