@@ -238,19 +238,26 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
     for (int m0 = 0; m0 <= SEG; m0 += NB) {
         double sp[NB], sm[NB];
         bool need = false, needB = false;
+        // High-word test of slopes_fast, once for the batch (conservative): every |d| of the batch below
+        // min(2 min f, 2 (f_inf - max f)) means every eps is 1.  Running integer min / max of the high words, one fp64
+        // subtraction per batch; comparisons, not differences (the high word of a bound is hugely negative for f < 0
+        // or f > f_inf: round-off leaves -1e-17 behind).
+        int hmin = 0x7fffffff, hmx = (int)0x80000000, dmax = LIM ? (__double2hiint(q[m0 + 1] - q[m0]) & 0x7fffffff) : 0;
 #pragma unroll
         for (int i = 0; i < NB; ++i) {
             const int m = m0 + i;
             if (m > SEG) break;
             const double f0 = q[m + 1];
             sp[i] = q[m + 2] - f0; sm[i] = f0 - q[m];
-            if (LIM) {   // high-word test of slopes_fast: may a bound bind (conservative)?  Comparisons, not differences:
-                         // hf, hg are hugely negative for f0 < 0 or f0 > f_inf (round-off leaves -1e-17 behind)
-                const int hf = __double2hiint(f0) + 0x00100000, hg = __double2hiint(finf - f0) + 0x00100000;
-                const int hmax = max(__double2hiint(sp[i]) & 0x7fffffff, __double2hiint(sm[i]) & 0x7fffffff);
-                need |= hmax >= min(hf, hg);
-                needB |= hmax >= hg;
+            if (LIM) {
+                hmin = min(hmin, __double2hiint(f0)); hmx = max(hmx, __double2hiint(f0));
+                dmax = max(dmax, __double2hiint(sp[i]) & 0x7fffffff);
             }
+        }
+        if (LIM) {
+            const int hg = __double2hiint(finf - __hiloint2double(hmx + 1, 0)) + 0x00100000;
+            need = dmax >= min(hmin + 0x00100000, hg);
+            needB = dmax >= hg;
         }
         // (without FULL the lanes voting together are whoever is here right now: the votes only decide which of two
         // equivalent evaluations runs, so any grouping that includes the lane itself is right)
