@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     } else if (P.axis == 2) {
         base = P.src + (long)other * P.S + v;
         obase = P.dst + (long)other * P.S + v;
-        vc = P.vmin + ((int)(v % P.nv2) + 0.5) * P.dv;      // VEC = 1: one v_z cell per thread
+        vc = P.vmin + ((int)(v % P.nv2) + 0.5) * P.dv;      // the first v_z cell of this thread
     } else {
         const long zo = (long)blockIdx.z * P.slab;
         base = P.src + zo + ((long)P.g * P.nx + other) * P.S + v;
@@ -112,11 +112,23 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     }
     const int N = P.n_line;
     const double sigma = vc * P.dts / P.dxx;
-    const int u = sigma >= 0.0 ? 1 : -1;
+    int u = sigma >= 0.0 ? 1 : -1;
     int n; double b;
     split_shift(fabs(sigma), n, b);
     const bool periodic = P.axis != 1 || (P.bc_lo == VLASOV_BC_PERIODIC && P.bc_hi == VLASOV_BC_PERIODIC);
     if (periodic) n %= N;
+    // shift fraction per packed cell: the same for both in x and y sweeps (sigma depends on i_vx / i_vy); in a z sweep
+    // the two v_z cells of a thread have their own sigma -- the launcher packs two only when every |sigma_z| < 1 and
+    // no pair straddles v_z = 0 (one direction, no whole cells)
+    double bv[VEC];
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) bv[e] = b;
+    if (VEC == 2 && P.axis == 2) {
+        const double s1 = (vc + P.dv) * P.dts / P.dxx;
+        u = sigma + s1 >= 0.0 ? 1 : -1;
+        n = 0;
+        bv[0] = fabs(sigma); bv[VEC - 1] = fabs(s1);
+    }
     bool bad = false;
 
     // march i = i0, i0+u, ...; source cell j = i - u n
@@ -128,7 +140,7 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     {
         Pack<VEC> fmm = fetch<VEC>(P, base, mir, j - 2 * u, bad);
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) Gp.v[e] = partial_flux(fmm.v[e], fm.v[e], f0.v[e], b, P.finf, P.limiter);
+        for (int e = 0; e < VEC; ++e) Gp.v[e] = partial_flux(fmm.v[e], fm.v[e], f0.v[e], bv[e], P.finf, P.limiter);
     }
     Pack<VEC> q[PF];
 #pragma unroll
@@ -143,7 +155,7 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
                 Pack<VEC> o;
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) {
-                    double G = partial_flux(fm.v[e], f0.v[e], fp.v[e], b, P.finf, P.limiter);
+                    double G = partial_flux(fm.v[e], f0.v[e], fp.v[e], bv[e], P.finf, P.limiter);
                     o.v[e] = f0.v[e] + (Gp.v[e] - G);      // eq. (38): f + (Phi_{i-1/2} - Phi_{i+1/2})
                     Gp.v[e] = G;
                 }
@@ -177,10 +189,21 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
     if (nrows < 0) nrows = G.nrows;              // x sweep: the rows of every z slab
     if (nrows == 0) return VLASOV_OK;
     const int threads = 128;
-    if (axis == 2) {                             // sigma depends on i_vz: one v_z cell per thread
-        dim3 grid((unsigned)((s.nvtot + threads - 1) / threads), (unsigned)(G.nyg * G.nx));
+    if (axis == 2) {                             // sigma depends on i_vz
+        // two v_z cells per thread (16-byte accesses) when both march the same way with no whole cells, else one
+        bool pack = true;
+        for (int k = 0; k + 1 < s.nv[2] && pack; k += 2) {
+            const double s0 = (s.vmin[2] + (k + 0.5) * s.dv[2]) * dts / G.dz, s1 = (s.vmin[2] + (k + 1.5) * s.dv[2]) * dts / G.dz;
+            pack = s0 * s1 >= 0.0 && fabs(s0) < 1.0 && fabs(s1) < 1.0;
+        }
         Launch L(c, K_SWEEP_Z);
-        sweep_space_kernel<1, 4><<<grid, threads, 0, c->stream>>>(P);
+        if (pack) {
+            dim3 grid((unsigned)((s.nvtot / 2 + threads - 1) / threads), (unsigned)(G.nyg * G.nx));
+            sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
+        } else {
+            dim3 grid((unsigned)((s.nvtot + threads - 1) / threads), (unsigned)(G.nyg * G.nx));
+            sweep_space_kernel<1, 4><<<grid, threads, 0, c->stream>>>(P);
+        }
     } else {
         const long chunks = s.nvtot / 2;
         dim3 grid((unsigned)((chunks + threads - 1) / threads), (unsigned)(axis == 0 ? nrows : G.nx), (unsigned)(axis == 0 ? 1 : G.nz));
