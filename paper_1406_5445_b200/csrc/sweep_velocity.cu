@@ -666,12 +666,15 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
 #ifndef VL_YZ40_PLANES
 #define VL_YZ40_PLANES 2
 #endif
-__host__ __device__ constexpr int yz_tma_planes(int cn) { return cn == 40 ? VL_YZ40_PLANES : 2048 / (cn * cn) > 0 ? 2048 / (cn * cn) : 1; }
+#ifndef VL_YZ32_PLANES
+#define VL_YZ32_PLANES 2
+#endif
+__host__ __device__ constexpr int yz_tma_planes(int cn) { return cn == 40 ? VL_YZ40_PLANES : cn == 32 ? VL_YZ32_PLANES : 2048 / (cn * cn) > 0 ? 2048 / (cn * cn) : 1; }
 __host__ __device__ constexpr int yz_tma_threads(int cn) { return (yz_tma_planes(cn) * cn * ((cn + 7) / 8) + 31) / 32 * 32; }
-static_assert(yz_tma_threads(32) == 256 && yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(48) == 288, "");
+static_assert(yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(48) == 288, "");
 // resident CTAs per SM the kernel is compiled for: 3 (80 registers at 256 threads); one 48x48 plane has 288 work items
 // (9 warps) and 69 KB of shared memory: 2 CTAs per SM
-__host__ __device__ constexpr int yz_tma_minb(int cn) { return cn == 48 || (cn == 40 && VL_YZ40_PLANES > 1) ? 2 : VL_YZ_MINB; }
+__host__ __device__ constexpr int yz_tma_minb(int cn) { return cn == 48 || (cn == 40 && VL_YZ40_PLANES > 1) ? 2 : cn == 32 && VL_YZ32_PLANES == 1 ? 6 : cn == 32 && VL_YZ32_PLANES == 4 ? 1 : VL_YZ_MINB; }
 
 // MOM = 1 (VXV order): the 10 raw velocity moments, eqs. (2)-(4), of the final f are
 // reduced in this kernel.  A CTA then takes WHOLE spatial cells (all tiles of a cell one after the other), sums its
