@@ -41,7 +41,8 @@ enum {
     VLASOV_EALIGN = -2,  /* a device pointer is not 128-byte aligned */
     VLASOV_ESHIFT = -3,  /* a y-shift reaches beyond the ghost rows of a FLUID side (R9) */
     VLASOV_EDOMAIN = -4, /* Boris denominator <= 0 (R13), or n<=0 / T<=0 / p<=0 in the ghost fill */
-    VLASOV_ECUDA = -5    /* a CUDA runtime call failed (or no device) */
+    VLASOV_ECUDA = -5,   /* a CUDA runtime call failed (or no device) */
+    VLASOV_ETOOBIG = -6  /* vlasov_fluid_step_static: the block needs more than VLASOV_FLUID_STATIC_SCRATCH_BYTES */
 };
 
 /* y-side kinds; x is always periodic (R16, R19). */
@@ -224,6 +225,24 @@ typedef struct {
 size_t vlasov_fluid_scratch_bytes(const vlasov_fluid_config* cfg);
 int vlasov_fluid_step(const vlasov_fluid_config* cfg, double dt, double* U_dev, const double* E_dev, const double* B_dev,
                       const double* ghost_lo_dev, const double* ghost_hi_dev, void* scratch_dev, size_t scratch_bytes);
+/* vlasov_fluid_step for callers that cannot allocate device memory (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the same step, same arguments and results bit for bit, with the two Runge-Kutta
+ * stage buffers in a file-scope `static __device__` array of the library instead of the caller's scratch_dev.  Calls no
+ * cudaMalloc, cudaFree or allocating library routine; the array (VLASOV_FLUID_STATIC_SCRATCH_BYTES = 4 MiB, aligned to
+ * 256 bytes) is part of the library image, so every GPU that loads the library holds it until the process exits.  Its
+ * device address is looked up once per device (cudaGetSymbolAddress with that device current) on the first call there:
+ * make one call per device outside any capture, with the device current that owns U_dev.
+ *   Limit: vlasov_fluid_scratch_bytes(cfg) <= VLASOV_FLUID_STATIC_SCRATCH_BYTES, i.e. nspecies * (ny + 4) * nx <= 52428
+ *   cells (e.g. 2 species on 256 x 98; the 256 x 48 blocks beside config 4's band need 2.1 MB); beyond it the call
+ *   returns VLASOV_ETOOBIG and launches nothing.
+ *   Sharing: every call on a device uses the same array, which keeps the last call's contents.  Nothing in it has to
+ *   start at zero (each stage buffer is written in full, ghost rows included, before it is read), so nothing is cleared.
+ *   Calls that overlap on the GPU (two streams, two host threads, this entry point inside two graphs that run
+ *   concurrently) RACE on the array: serialise them, or use vlasov_fluid_step with scratch of your own.
+ * Errors: those of vlasov_fluid_step, and ETOOBIG. */
+#define VLASOV_FLUID_STATIC_SCRATCH_BYTES (4u << 20)
+int vlasov_fluid_step_static(const vlasov_fluid_config* cfg, double dt, double* U_dev, const double* E_dev,
+                             const double* B_dev, const double* ghost_lo_dev, const double* ghost_hi_dev);
 /* eqs. (2)-(4) PAPER.md:39-46: rho = m M0, u = m M1, energy = (m/2)(M2xx + M2yy + M2zz) from raw moments [10][n] (the
  * layout of vlasov_moments / vlasov_fluid_boundary) to fluid variables [5][n]. */
 int vlasov_fluid_from_moments(const double* mom10_dev, double m, double* U5_dev, long n, void* stream);

@@ -11,7 +11,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 # VLASOV_B200_LIB: another build of the same library (A/B measurements of kernel variants); default: the in-tree build
 LIB_PATH = os.environ.get("VLASOV_B200_LIB") or os.path.join(HERE, "libvlasov_b200.so")
 
-OK, EINVAL, EALIGN, ESHIFT, EDOMAIN, ECUDA = 0, -1, -2, -3, -4, -5
+OK, EINVAL, EALIGN, ESHIFT, EDOMAIN, ECUDA, ETOOBIG = 0, -1, -2, -3, -4, -5, -6
+FLUID_STATIC_SCRATCH_BYTES = 4 << 20
 BC_PERIODIC, BC_REFLECT, BC_FLUID = 0, 1, 2
 ORDER_XVX, ORDER_VXV = 0, 1
 STAGE_X1, STAGE_V, STAGE_X2, STAGE_GHOST, STAGE_MOMENTS, STAGE_ALL = 1, 2, 4, 8, 16, 31
@@ -20,7 +21,8 @@ EXPORTS = ["vlasov_scratch_bytes", "vlasov_init", "vlasov_set_boundary", "vlasov
            "vlasov_moments", "vlasov_current", "vlasov_maxwell", "vlasov_touch", "vlasov_set_option", "vlasov_check",
            "vlasov_launch_count", "vlasov_free", "vlasov_strerror", "vlasov_cycle", "vlasov_cycle_host",
            "vlasov_timing_enable", "vlasov_timing_read", "vlasov_fluid_boundary_mark", "vlasov_fluid_boundary",
-           "vlasov_fluid_scratch_bytes", "vlasov_fluid_step", "vlasov_fluid_from_moments", "vlasov_fluid_to_boundary"]
+           "vlasov_fluid_scratch_bytes", "vlasov_fluid_step", "vlasov_fluid_from_moments", "vlasov_fluid_to_boundary",
+           "vlasov_fluid_step_static"]
 FLUID_BC_PERIODIC, FLUID_BC_WALL, FLUID_BC_COUPLED = 0, 1, 2
 OPT_FUSE_XY = 1
 OPT_FUSE_MOMENTS = 2
@@ -109,6 +111,8 @@ def lib():
         L.vlasov_fluid_scratch_bytes.argtypes = [C.POINTER(vlasov_fluid_config)]
         L.vlasov_fluid_step.restype = C.c_int
         L.vlasov_fluid_step.argtypes = [C.POINTER(vlasov_fluid_config), C.c_double, dp, dp, dp, dp, dp, vp, C.c_size_t]
+        L.vlasov_fluid_step_static.restype = C.c_int
+        L.vlasov_fluid_step_static.argtypes = [C.POINTER(vlasov_fluid_config), C.c_double, dp, dp, dp, dp, dp]
         L.vlasov_fluid_from_moments.restype = C.c_int
         L.vlasov_fluid_from_moments.argtypes = [dp, C.c_double, dp, C.c_long, vp]
         L.vlasov_fluid_to_boundary.restype = C.c_int
@@ -298,6 +302,11 @@ class FluidBlock:
     def vlasov_fluid_step(self, dt, U, E, B, ghost_lo=None, ghost_hi=None):
         _chk(lib().vlasov_fluid_step(C.byref(self.cfg), float(dt), _ptr(U), _ptr(E), _ptr(B), _ptr(ghost_lo), _ptr(ghost_hi),
                                      C.c_void_p(self.scratch.data_ptr()), C.c_size_t(self.scratch.numel())), "vlasov_fluid_step")
+
+    def vlasov_fluid_step_static(self, dt, U, E, B, ghost_lo=None, ghost_hi=None):
+        """The same step with the stage buffers in the library's static device array: no allocation (include/vlasov.h)."""
+        _chk(lib().vlasov_fluid_step_static(C.byref(self.cfg), float(dt), _ptr(U), _ptr(E), _ptr(B), _ptr(ghost_lo),
+                                            _ptr(ghost_hi)), "vlasov_fluid_step_static")
 
 
 def vlasov_fluid_from_moments(mom10, m, U5, stream=None):

@@ -450,6 +450,7 @@ const char* vlasov_strerror(int err) {
         case VLASOV_ESHIFT: return "y shift reaches beyond the ghost rows";
         case VLASOV_EDOMAIN: return "Boris denominator or ghost-fill moment out of domain";
         case VLASOV_ECUDA: return "CUDA runtime error or no device";
+        case VLASOV_ETOOBIG: return "fluid block larger than the static scratch array (VLASOV_FLUID_STATIC_SCRATCH_BYTES)";
         default: return "unknown error";
     }
 }

@@ -11,6 +11,7 @@
 // (section 4.1: "boundary conditions at times t, t + dt/2 and t + dt").
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <atomic>
 #include "../../include/vlasov.h"
 
 namespace vlf {
@@ -205,3 +206,36 @@ int vlasov_fluid_to_boundary(const double* U5_dev, double m, double* fluid5_dev,
 }
 
 }  // extern "C"
+
+// ---- vlasov_fluid_step without an allocation anywhere (include/vlasov.h) ---------------------------------------------
+// The two stage buffers live in the library image.  In host code `fluid_static_scratch` is a host-side stand-in, not a
+// device address: the address a kernel may use comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char fluid_static_scratch[VLASOV_FLUID_STATIC_SCRATCH_BYTES];
+
+namespace vlf {
+
+constexpr int MAX_DEVICES = 64;
+std::atomic<void*> static_scratch_addr[MAX_DEVICES];      // zero-initialised; one slot per device ordinal
+
+// device address of fluid_static_scratch on the current device (nullptr on a CUDA error)
+static void* static_scratch_of_current_device() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return nullptr;
+    void* p = static_scratch_addr[dev].load(std::memory_order_acquire);
+    if (p) return p;
+    if (cudaGetSymbolAddress(&p, fluid_static_scratch) != cudaSuccess || !p) return nullptr;
+    static_scratch_addr[dev].store(p, std::memory_order_release);     // same value whoever gets here first
+    return p;
+}
+
+}  // namespace vlf
+
+extern "C" int vlasov_fluid_step_static(const vlasov_fluid_config* cfg, double dt, double* U_dev, const double* E_dev,
+                                        const double* B_dev, const double* ghost_lo_dev, const double* ghost_hi_dev) {
+    const size_t need = vlasov_fluid_scratch_bytes(cfg);
+    if (!need) return VLASOV_EINVAL;
+    if (need > (size_t)VLASOV_FLUID_STATIC_SCRATCH_BYTES) return VLASOV_ETOOBIG;
+    void* scratch = vlf::static_scratch_of_current_device();
+    if (!scratch) return VLASOV_ECUDA;
+    return vlasov_fluid_step(cfg, dt, U_dev, E_dev, B_dev, ghost_lo_dev, ghost_hi_dev, scratch, need);
+}
