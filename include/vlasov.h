@@ -37,7 +37,7 @@ typedef struct vlasov_ctx vlasov_ctx; /* opaque */
 
 enum {
     VLASOV_OK = 0,
-    VLASOV_EINVAL = -1,  /* bad argument (null pointer, non-positive size, odd nvz, unknown enum) */
+    VLASOV_EINVAL = -1,  /* bad argument (null pointer, non-positive size, unknown enum) */
     VLASOV_EALIGN = -2,  /* a device pointer is not 128-byte aligned */
     VLASOV_ESHIFT = -3,  /* a y-shift reaches beyond the ghost rows of a FLUID side (R9) */
     VLASOV_EDOMAIN = -4, /* Boris denominator <= 0 (R13), or n<=0 / T<=0 / p<=0 in the ghost fill */
@@ -64,7 +64,7 @@ enum {
 
 typedef struct {
     double q, m;       /* charge and mass, eq. (1) */
-    int32_t nv[3];     /* velocity cells per direction; nv[2] must be even */
+    int32_t nv[3];     /* velocity cells per direction (any; an even nv[2] takes the 16-byte paths) */
     double vmin[3];    /* lower faces of the velocity box; centres vmin + (k+1/2) dv */
     double vmax[3];    /* upper faces */
     double f_inf;      /* f_infinity of eqs. (43),(44) PAPER.md:273-276 (R6): a per-species constant > 0 */

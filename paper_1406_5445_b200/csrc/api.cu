@@ -21,7 +21,7 @@ bool carve(const vlasov_config* cfg, const vlasov_species* sp, Carve& C) {
     const size_t ncell = nyg * cfg->nx * (size_t)(cfg->nz > 1 ? cfg->nz : 1);
     size_t maxS = 0;
     for (int s = 0; s < cfg->nspecies; ++s) {
-        if (sp[s].nv[0] <= 0 || sp[s].nv[1] <= 0 || sp[s].nv[2] <= 0 || (sp[s].nv[2] & 1)) return false;
+        if (sp[s].nv[0] <= 0 || sp[s].nv[1] <= 0 || sp[s].nv[2] <= 0) return false;
         size_t S = (size_t)sp[s].nv[0] * sp[s].nv[1] * sp[s].nv[2];
         if (S > maxS) maxS = S;
     }

@@ -21,32 +21,47 @@ struct MomParams {
 
 constexpr int MOM_THREADS = 256;
 
+// VEC = 2: a thread owns pairs of neighbouring v_z cells (16-byte loads; nv[2] even).  VEC = 1: one column per thread
+// (any nv[2]); the same sums in the same order per column.
+template <int VEC>
 __global__ void __launch_bounds__(MOM_THREADS) moments_kernel(MomParams P) {
     const int cell = P.cell0 + blockIdx.x;
     const double* fb = P.f + (long)cell * P.S;
     const int plane = P.nv1 * P.nv2;
-    const int nchunk = plane / 2;
+    const int nchunk = plane / VEC;
     double M[10];
 #pragma unroll
     for (int k = 0; k < 10; ++k) M[k] = 0.0;
     double mx = 0.0;
     for (int ch = threadIdx.x; ch < nchunk; ch += MOM_THREADS) {
-        const int col = 2 * ch;
+        const int col = VEC * ch;
         const int iy = col / P.nv2, iz = col - iy * P.nv2;
         const double vy = P.vmin[1] + (iy + 0.5) * P.dv[1];
         const double vza = P.vmin[2] + (iz + 0.5) * P.dv[2];
         const double vzb = P.vmin[2] + (iz + 1.5) * P.dv[2];
         double a0 = 0, a1 = 0, a2 = 0, b0 = 0, b1 = 0, b2 = 0;
-        const double2* p = reinterpret_cast<const double2*>(fb + col);
-        const long pstride = plane / 2;
+        if constexpr (VEC == 2) {
+            const double2* p = reinterpret_cast<const double2*>(fb + col);
+            const long pstride = plane / 2;
 #pragma unroll 4
-        for (int k = 0; k < P.nv0; ++k) {
-            const double vx = P.vmin[0] + (k + 0.5) * P.dv[0];
-            const double2 v = __ldcs(p + (long)k * pstride);
-            const double wa = vx * v.x, wb = vx * v.y;
-            a0 += v.x; a1 += wa; a2 += vx * wa;
-            b0 += v.y; b1 += wb; b2 += vx * wb;
-            mx = fmax(mx, fmax(v.x, v.y));
+            for (int k = 0; k < P.nv0; ++k) {
+                const double vx = P.vmin[0] + (k + 0.5) * P.dv[0];
+                const double2 v = __ldcs(p + (long)k * pstride);
+                const double wa = vx * v.x, wb = vx * v.y;
+                a0 += v.x; a1 += wa; a2 += vx * wa;
+                b0 += v.y; b1 += wb; b2 += vx * wb;
+                mx = fmax(mx, fmax(v.x, v.y));
+            }
+        } else {
+            const double* p = fb + col;
+#pragma unroll 4
+            for (int k = 0; k < P.nv0; ++k) {
+                const double vx = P.vmin[0] + (k + 0.5) * P.dv[0];
+                const double v = __ldcs(p + (long)k * plane);
+                const double wa = vx * v;
+                a0 += v; a1 += wa; a2 += vx * wa;
+                mx = fmax(mx, v);
+            }
         }
         const double s0 = a0 + b0, s1 = a1 + b1, s2 = a2 + b2;
         const double z0 = vza * a0 + vzb * b0;          // sum vz f
@@ -96,7 +111,8 @@ int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out
     P.ncell_out = nrows * c->G.nx;
     {
         Launch L(c, K_MOMENTS);
-        moments_kernel<<<P.ncell_out, MOM_THREADS, 0, c->stream>>>(P);
+        if (s.nv[2] % 2 == 0) moments_kernel<2><<<P.ncell_out, MOM_THREADS, 0, c->stream>>>(P);
+        else moments_kernel<1><<<P.ncell_out, MOM_THREADS, 0, c->stream>>>(P);
     }
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }

@@ -191,7 +191,7 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
     const int threads = 128;
     if (axis == 2) {                             // sigma depends on i_vz
         // two v_z cells per thread (16-byte accesses) when both march the same way with no whole cells, else one
-        bool pack = true;
+        bool pack = s.nv[2] % 2 == 0;
         for (int k = 0; k + 1 < s.nv[2] && pack; k += 2) {
             const double s0 = (s.vmin[2] + (k + 0.5) * s.dv[2]) * dts / G.dz, s1 = (s.vmin[2] + (k + 1.5) * s.dv[2]) * dts / G.dz;
             pack = s0 * s1 >= 0.0 && fabs(s0) < 1.0 && fabs(s1) < 1.0;
@@ -205,10 +205,13 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
             sweep_space_kernel<1, 4><<<grid, threads, 0, c->stream>>>(P);
         }
     } else {
-        const long chunks = s.nvtot / 2;
+        // two neighbouring v_z cells per thread (one sigma, one wall image, 16-byte accesses) need an even nv[2]
+        const bool pack = s.nv[2] % 2 == 0;
+        const long chunks = pack ? s.nvtot / 2 : s.nvtot;
         dim3 grid((unsigned)((chunks + threads - 1) / threads), (unsigned)(axis == 0 ? nrows : G.nx), (unsigned)(axis == 0 ? 1 : G.nz));
         Launch L(c, axis == 0 ? K_SWEEP_X : K_SWEEP_Y);
-        sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
+        if (pack) sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
+        else sweep_space_kernel<1, 4><<<grid, threads, 0, c->stream>>>(P);
     }
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }

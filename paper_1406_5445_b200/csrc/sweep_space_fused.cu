@@ -399,7 +399,8 @@ static bool pick_xy_shape(const Geom& G, const Species& s, int& xb, int& C) {
     if (G.nx % 4 == 0) xb = 4;
     const int nblk = G.nx / xb;
     C = 32;
-    auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && nblk * cc <= VL_XY_MAXT; };
+    // (a piece = min(cc, nv[2]) cells is one TMA box row: at least 16 bytes, so an odd nv[2] has no shape here)
+    auto ok = [&](int cc) { return s.nvtot % cc == 0 && (s.nv[2] % cc == 0 || cc % s.nv[2] == 0) && s.nv[2] >= 2 && nblk * cc <= VL_XY_MAXT; };
     while (C >= 2 && !ok(C)) C >>= 1;
     if (C < 2) return false;
     if (xy_box_rows(G.nx) == 0) return false;      // no equal split of a row into TMA boxes of at most 256 x cells

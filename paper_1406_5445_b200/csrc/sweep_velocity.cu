@@ -463,11 +463,18 @@ __global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams
         const double t0 = T[0], t1 = T[1], t2 = T[2], t3 = T[3], finf = T[12], scale = T[15];
         const double* fsrc = P.fsrc + (long)T[16] * P.S + c0;
         double* fb = P.f + (long)cell * P.S + c0;
-        for (int e = threadIdx.x; e < N * H; e += V_THREADS) {
-            const int k = e / H, c = 2 * (e - k * H);
-            double2 v = make_double2(0.0, 0.0);
-            if (c < ncol) { v = __ldcs(reinterpret_cast<const double2*>(fsrc + (long)k * plane + c)); v.x *= scale; v.y *= scale; }
-            *reinterpret_cast<double2*>(A + k * CT + c) = v;
+        if (CN || !(plane & 1)) {      // pairs of columns by 16-byte loads: every row of the tile starts on an even cell
+            for (int e = threadIdx.x; e < N * H; e += V_THREADS) {
+                const int k = e / H, c = 2 * (e - k * H);
+                double2 v = make_double2(0.0, 0.0);
+                if (c < ncol) { v = __ldcs(reinterpret_cast<const double2*>(fsrc + (long)k * plane + c)); v.x *= scale; v.y *= scale; }
+                *reinterpret_cast<double2*>(A + k * CT + c) = v;
+            }
+        } else {                       // nv[1] nv[2] odd: column by column
+            for (int e = threadIdx.x; e < N * CT; e += V_THREADS) {
+                const int k = e / CT, c = e - k * CT;
+                A[k * CT + c] = c < ncol ? __ldcs(fsrc + (long)k * plane + c) * scale : 0.0;
+            }
         }
         __syncthreads();
         for (int wi = threadIdx.x; wi < CT * nsegx; wi += V_THREADS) {

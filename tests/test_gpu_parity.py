@@ -256,6 +256,31 @@ def test_velocity_step_moderate_rotation(gpu, orc, limiter, nv):
 
 
 @pytest.mark.parametrize("order", [0, 1])
+@pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_REFLECT])
+@pytest.mark.parametrize("nv,dt", [((6, 5, 7), 0.07), ((5, 3, 3), 0.07), ((4, 4, 5), 0.23), ((8, 6, 9), 0.02), ((6, 4, 1), 0.07)])
+def test_full_step_odd_velocity_grids(gpu, orc, order, bc, nv, dt):
+    """Velocity grids with an odd nv[2] (and an odd block, 5x3x3; a single v_z cell, 6x4x1): nothing in the method asks
+    for an even count, only the 16-byte paths of the kernels do -- these shapes take one cell per thread in the spatial
+    sweeps and the moments and column-by-column tile loads in the vx sweep.  dt = 0.02: all spatial shifts below one
+    cell (the fused stage has no shape for an odd nv[2]: the general kernels run); 0.23: multi-cell shifts."""
+    rng = np.random.default_rng(17)
+    w = random_workload(rng, nx=7, ny=5, nv=nv, bc=bc, nspecies=2, fields_yee=1)
+    f0 = [smooth_random_f(rng, w, s) for s in range(2)]
+    E = rng.standard_normal((3, w.ny_g, w.nx))
+    B = 2.0 * rng.standard_normal((3, w.ny_g, w.nx))
+    fg, fo, mg, mo, code = run_both(gpu, orc, w, f0, E, B, dt, 31, order=order)
+    assert code == 0
+    assert run_both.kinds["sweep_xy"][1] + run_both.kinds["sweep_yx"][1] == 0
+    for s in range(2):
+        assert rel_l2(fg[s], fo[s]) <= TOL1
+        assert np.abs(fg[s] - fo[s]).max() <= 2e-13
+        assert rel_l2(mg[s], mo[s]) <= TOL1
+        m0 = f0[s].sum()
+        assert abs(fg[s].sum() - m0) / m0 <= 1e-13
+        assert np.abs(fg[s] - f0[s]).max() > 0.05
+
+
+@pytest.mark.parametrize("order", [0, 1])
 @pytest.mark.parametrize("limiter", [1, 0])
 def test_full_step_two_species(gpu, orc, order, limiter):
     rng = np.random.default_rng(3)
@@ -290,9 +315,10 @@ def test_gem_cut_one_step(gpu, orc):
         assert abs(fg[s].sum() - m0) / m0 <= 1e-13
 
 
-@pytest.mark.parametrize("nx,ny_band,nv", [(16, 8, 16), (16, 32, 40)])
+@pytest.mark.parametrize("nx,ny_band,nv", [(16, 8, 16), (16, 32, 40), (8, 8, 15)])
 def test_ghost_fill_band(gpu, orc, nx, ny_band, nv):
-    """a0 on a cut of config 4: FLUID sides, 3 ghost rows, seeded fluid state; ghost rows and interior.  (16, 32, 40) is
+    """a0 on a cut of config 4: FLUID sides, 3 ghost rows, seeded fluid state; ghost rows and interior.  15^3: an odd
+    velocity block (column-by-column tile loads, one v_z column per thread in the moments).  (16, 32, 40) is
     SURVEY 8(d) config 4's "16x32 x-cut" at the real 40^3 velocity grid: there the ghost fill takes the general vx
     kernel in ghost mode (scale T[15], source cell T[16]) and the 40x40-plane vy+vz kernel."""
     w = inputs.band_workload(nx=nx, ny_band=ny_band, ny_domain=128, nv=nv, g=3)
