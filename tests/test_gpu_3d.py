@@ -180,3 +180,52 @@ def test_3d_refusals(gpu):
     with pytest.raises(gpu.VlasovError) as e:
         gpu.context_for(w, f)                       # ghost rows (FLUID sides) are a 2D3V feature
     assert e.value.code == gpu.EINVAL
+
+
+def test_full_size_gem3d_sampled_window(gpu, orc):
+    """The 3D3V bench workload at full size (32x32x8 spatial x 32^3 velocity x 2 species, 4.3 GB of f), as
+    `bench.py --workload gem3d` runs it: one complete step on the GPU, then the oracle on a 14x14 window in x, y (all 8
+    z slabs: z is periodic) of the same inputs; the inner 4x4 columns must agree (domain of dependence of a step: 4
+    cells in x and y).  Mass and positivity at full size."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 9 * 2**30:
+        pytest.skip("needs 9 GB of device memory")
+    w = inputs.gem3d_workload(steps=1)
+    ix0, iy0, nw, margin = 9, 9, 14, 5
+    E, B = inputs.gem3d_fields(w)
+    fg, f0win, mass0 = [], [], []
+    for s, sp in enumerate(w.species):
+        sp.f_inf = inputs.gem_f_inf(w, s)
+        f = torch.empty((w.nz, w.ny, w.nx) + tuple(sp.nv), dtype=torch.float64, device="cuda")
+        win = np.empty((w.nz, nw, nw) + tuple(sp.nv))
+        for k in range(w.nz):
+            slab = inputs.gem3d_f(w, s, k)
+            f[k].copy_(torch.from_numpy(slab))
+            win[k] = slab[iy0:iy0 + nw, ix0:ix0 + nw]
+        fg.append(f)
+        f0win.append(win)
+        mass0.append(float(f.sum().item()))
+    ctx = gpu.context_for(w, fg)
+    ctx.vlasov_timing_enable(True)
+    ctx.vlasov_step(w.dt, dev(E), dev(B), gpu.STAGE_ALL)
+    assert ctx.check_code() == 0
+    kinds = ctx.vlasov_timing_read()
+    assert kinds["sweep_xy"][1] == 2 and kinds["sweep_yx"][1] == 2 and kinds["sweep_z"][1] == 4 and kinds["vsweep_yz"][1] == 2
+    Ew = np.ascontiguousarray(E[:, :, iy0:iy0 + nw, ix0:ix0 + nw])
+    Bw = np.ascontiguousarray(B[:, :, iy0:iy0 + nw, ix0:ix0 + nw])
+    inner = slice(margin, nw - margin)
+    for s, sp in enumerate(w.species):
+        drift = abs(float(fg[s].sum().item()) - mass0[s]) / mass0[s]
+        assert drift <= 1e-13, (s, drift)
+        assert float(fg[s].min().item()) >= 0.0
+        fo = f0win[s].copy()
+        err, _ = orc.step3d(fo, osp(orc, sp), nw, nw, w.nz, nw * w.dx, nw * w.dy, w.lz, w.dt, Ew, Bw, fields_yee=w.fields_yee,
+                            bc_lo=inputs.BC_PERIODIC, bc_hi=inputs.BC_PERIODIC, order=0, want_moments=False)
+        assert err == 0
+        got = fg[s][:, iy0:iy0 + nw, ix0:ix0 + nw].cpu().numpy()
+        a, b = got[:, inner, inner], fo[:, inner, inner]
+        assert rel(a, b) <= TOL1, s
+        assert np.abs(a - b).max() <= 1e-13 * sp.f_inf
+        assert rel(got[:, 0], fo[:, 0]) > 1e-9          # the window's own edge does differ: not vacuous
+    ctx.close()

@@ -595,6 +595,93 @@ def test_full_size_gem128_sampled_window(gpu, orc):
     ctx.close()
 
 
+def _full_size_window(gpu, orc, w, ix0, nw, iy0=None, margin=5, fluid=None, expect=None, need_gb=9):
+    """One complete step of workload w at full size on the GPU (as bench.py runs it), then the oracle on the spatial
+    window [iy0, iy0 + nw) x [ix0, ix0 + nw) of the same inputs (iy0 None: every row, ghost rows included, with the
+    workload's own y boundaries); cells at least `margin` from the window's artificial edges must agree (domain of
+    dependence of a step: 4 cells per direction).  Also the properties that hold at any size: mass, f >= 0 up to rounding
+    (periodic or wall sides only: ghost fills are not conservative)."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < need_gb * 2**30:
+        pytest.skip(f"needs {need_gb} GB of device memory")
+    rows = range(w.ny_g) if iy0 is None else range(iy0, iy0 + nw)
+    E, B = inputs.gem_fields(w)
+    fg, f0win, mass0 = [], [], []
+    for s, sp in enumerate(w.species):
+        sp.f_inf = inputs.gem_f_inf(w, s)
+        f = torch.empty((w.ny_g, w.nx) + tuple(sp.nv), dtype=torch.float64, device="cuda")
+        win = np.empty((len(rows), nw) + tuple(sp.nv))
+        for r in range(w.ny_g):
+            row = inputs.gem_f(w, s, rows=[r])[0]
+            f[r].copy_(torch.from_numpy(row))
+            if r in rows:
+                win[r - rows[0]] = row[ix0:ix0 + nw]
+        fg.append(f)
+        f0win.append(win)
+        mass0.append(float(f.sum().item()))
+    ctx = gpu.context_for(w, fg)
+    keep = []
+    if fluid is not None:
+        for s in range(len(w.species)):
+            for side in (0, 1):
+                keep.append(dev(fluid[s][side]))
+                ctx.vlasov_set_boundary(s, side, inputs.BC_FLUID, keep[-1])
+    ctx.vlasov_timing_enable(True)
+    Ed, Bd = dev(E), dev(B)
+    ctx.vlasov_step(w.dt, Ed, Bd, gpu.STAGE_ALL)
+    assert ctx.check_code() == 0
+    kinds = ctx.vlasov_timing_read()
+    for k, n in (expect or {}).items():
+        assert kinds[k][1] == n, (k, kinds[k])
+    ys = slice(None) if iy0 is None else slice(iy0, iy0 + nw)
+    Ew = np.ascontiguousarray(E[:, ys, ix0:ix0 + nw])
+    Bw = np.ascontiguousarray(B[:, ys, ix0:ix0 + nw])
+    inner_x = slice(margin, nw - margin)
+    inner_y = slice(None) if iy0 is None else slice(margin, nw - margin)
+    for s, sp in enumerate(w.species):
+        if fluid is None:
+            drift = abs(float(fg[s].sum().item()) - mass0[s]) / mass0[s]
+            assert drift <= 1e-13, (s, drift)
+            # eq. (38) forms f + (Phi - Phi): a cell that empties is left with a rounding residue of its neighbours' size
+            assert float(fg[s].min().item()) >= -1e-15 * sp.f_inf
+        fo = f0win[s].copy()
+        if iy0 is None:
+            fl = (None, None) if fluid is None else tuple(np.ascontiguousarray(fluid[s][side][:, :, ix0:ix0 + nw]) for side in (0, 1))
+            err, _ = orc.step(fo, osp(orc, sp), nw, w.ny, w.nghost_y, nw * w.dx, w.ly, w.dt, Ew, Bw, fields_yee=w.fields_yee,
+                              bc_lo=w.bc_y_lo, bc_hi=w.bc_y_hi, fluid_lo=fl[0], fluid_hi=fl[1], want_moments=False)
+        else:
+            err, _ = orc.step(fo, osp(orc, sp), nw, nw, 0, nw * w.dx, nw * w.dy, w.dt, Ew, Bw, fields_yee=w.fields_yee,
+                              bc_lo=inputs.BC_PERIODIC, bc_hi=inputs.BC_PERIODIC, want_moments=False)
+        assert err == 0
+        got = fg[s][ys, ix0:ix0 + nw].cpu().numpy()
+        assert rel_l2(got[inner_y, inner_x], fo[inner_y, inner_x]) <= TOL1, s
+        assert np.abs(got[inner_y, inner_x] - fo[inner_y, inner_x]).max() <= 1e-13 * sp.f_inf
+        tail_check(got[inner_y, inner_x], fo[inner_y, inner_x], what=f"{w.name} window, species {s}")
+        assert rel_l2(got[:, 0], fo[:, 0]) > 1e-9          # the window's own edge does differ: not vacuous
+    ctx.close()
+
+
+@pytest.mark.parametrize("nv", [48, 24, 16])
+def test_full_size_velocity_resolution_sweep_sampled_window(gpu, orc, nv):
+    """Config 5 (64x64 x nv^3 x 2 species) at full size, as `bench.py --workload nv48 | nv24 | nv16` runs it: persistent
+    velocity kernels with many tiles per CTA on 48x48 / 24x24 / 16x16 planes, the compile-time-shape fused stages."""
+    w = inputs.gem_workload(nx=64, ny=64, nv=nv, steps=1)
+    _full_size_window(gpu, orc, w, ix0=24, nw=16, iy0=24,
+                      expect={"sweep_xy": 2, "sweep_yx": 2, "vsweep_yz": 2, "vsweep_x": 2, "sweep_x": 0, "sweep_y": 0},
+                      need_gb=14 if nv == 48 else 4)
+
+
+def test_full_size_band_sampled_window(gpu, orc):
+    """Config 4 at full size (256 x 32 band + 3 FLUID ghost rows per side, 40^3, 2 species; 10 GB of f) as
+    `bench.py --workload band` runs it: ghost fill, fused stages on the interior, x sweeps of the ghost rows.  The oracle
+    advances every row of a 16-column cut with the same fluid state; its inner 6 columns must agree, ghost rows included."""
+    w = inputs.band_workload()
+    fluid = [[inputs.band_fluid_state(w, s, side, 0) for side in (0, 1)] for s in range(2)]
+    _full_size_window(gpu, orc, w, ix0=100, nw=16, iy0=None, fluid=fluid,
+                      expect={"sweep_xy": 2, "sweep_yx": 2, "ghost_vsweep_yz": 4, "ghost_sweep_x": 8, "sweep_y": 0}, need_gb=18)
+
+
 def test_gem_cut_50_cycles(gpu, orc):
     """north_star's long bar on a cut of config 2 (GEM Harris sheet, both species, 50 steps): 50 full cycles of
     section 4.3 (currents -> Maxwell half step -> Vlasov step -> currents -> Maxwell half step) through vlasov_cycle
