@@ -67,7 +67,8 @@ typedef struct {
     int32_t nv[3];     /* velocity cells per direction (any; an even nv[2] takes the 16-byte paths) */
     double vmin[3];    /* lower faces of the velocity box; centres vmin + (k+1/2) dv */
     double vmax[3];    /* upper faces */
-    double f_inf;      /* f_infinity of eqs. (43),(44) PAPER.md:273-276 (R6): a per-species constant > 0 */
+    double f_inf;      /* f_infinity of eqs. (43),(44) PAPER.md:273-276 (R6): a per-species upper bound of f, > 0;
+                          <= 0: vlasov_init takes max f of the species' f_dev as it stands (one pass, synchronises) */
 } vlasov_species;
 
 typedef struct {

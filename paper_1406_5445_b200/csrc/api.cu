@@ -169,7 +169,7 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     for (int s = 0; s < cfg->nspecies; ++s) {
         if (!f_dev[s]) return VLASOV_EINVAL;
         if (((uintptr_t)f_dev[s]) & 127) return VLASOV_EALIGN;
-        if (!(sp[s].m > 0.0) || !(sp[s].f_inf > 0.0)) return VLASOV_EINVAL;
+        if (!(sp[s].m > 0.0) || !(sp[s].f_inf == sp[s].f_inf)) return VLASOV_EINVAL;
         for (int d = 0; d < 3; ++d) if (!(sp[s].vmax[d] > sp[s].vmin[d])) return VLASOV_EINVAL;
         // a REFLECT wall builds its image by mirroring the i_vy index (R19): that is f(-vy) only on a symmetric vy grid
         if (cfg->bc_y_lo == VLASOV_BC_REFLECT || cfg->bc_y_hi == VLASOV_BC_REFLECT) {
@@ -226,6 +226,16 @@ int vlasov_init(const vlasov_config* cfg, const vlasov_species* sp, double* cons
     c->h_err = nullptr;
     if (cudaMallocHost((void**)&c->h_err, sizeof(int)) != cudaSuccess) { delete c; return VLASOV_ECUDA; }
     if (cudaMemsetAsync(c->errflag, 0, 128, c->stream) != cudaSuccess) { cudaFreeHost(c->h_err); delete c; return VLASOV_ECUDA; }
+    // f_inf <= 0: "take max f at init" (reading R6: f_infinity is an upper bound of f) -- one reduction
+    // pass over the species' f as it stands now
+    for (int s = 0; s < c->ns; ++s) {
+        if (c->sp[s].f_inf > 0.0) continue;
+        double mx = 0.0;
+        const int e = species_max_f(c, c->sp[s], &mx);
+        if (e || !(mx > 0.0)) { cudaFreeHost(c->h_err); delete c; return e ? e : VLASOV_EINVAL; }
+        c->sp[s].f_inf = mx;
+    }
+    c->launches = 0;
     *out = c;
     return VLASOV_OK;
 }

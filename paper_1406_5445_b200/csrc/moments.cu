@@ -117,6 +117,31 @@ int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
 
+// max over an array (one block; fmax is exact, so the order does not matter): f_infinity := max f at init (R6)
+__global__ void __launch_bounds__(256) max_kernel(const double* __restrict__ a, long n, double* __restrict__ out) {
+    __shared__ double red[256];
+    double m = a[0];
+    for (long i = threadIdx.x; i < n; i += 256) m = fmax(m, a[i]);
+    red[threadIdx.x] = m;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] = fmax(red[threadIdx.x], red[threadIdx.x + o]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = red[0];
+}
+
+// max of f over every cell of one species, through the 11th output of the moments kernel; synchronises the stream
+int species_max_f(vlasov_ctx* c, const Species& s, double* result) {
+    const int ncell = c->G.nrows * c->G.nx;
+    int e = launch_moments(c, s, s.f, c->mom, 0, c->G.nrows);
+    if (e) return e;
+    max_kernel<<<1, 256, 0, c->stream>>>(c->mom + (long)10 * ncell, ncell, c->gmom);
+    if (cudaMemcpyAsync(result, c->gmom, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return VLASOV_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return VLASOV_ECUDA;
+    return VLASOV_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Section 4.1: "by linear interpolation in time": out = (1 - theta) a + theta b, two products and a
 // sum, each rounded (no contraction), as the oracle writes it.

@@ -118,6 +118,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
                    double* mom_out = nullptr, bool* mom_done = nullptr, const double* src = nullptr);
 // moments (a9): out[11][nyg*nx] (10 moments + max f) of rows [row0,row0+nrows) of f
 int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out, int row0, int nrows);
+int species_max_f(vlasov_ctx* c, const Species& s, double* result);      // max f over all cells (synchronises)
 // ghost fill (a0) of one side
 int launch_ghost_fill(vlasov_ctx* c, const Species& s, double* f, int side);
 int launch_lerp(vlasov_ctx* c, const double* a, const double* b, double theta, double* out, long n);

@@ -832,6 +832,41 @@ def test_init_and_step_refusals(gpu):
     ctx.close()
 
 
+@pytest.mark.parametrize("nv", [(8, 8, 8), (6, 5, 7)])
+def test_f_inf_taken_from_the_data_at_init(gpu, orc, nv):
+    """f_inf <= 0 asks vlasov_init for max f of the data as it stands (reading R6): the step must then be the
+    oracle's with f_inf = max f of each species -- on data that does touch its upper bound (cells at the maximum next
+    to empty ones), so a wrong f_inf shows."""
+    rng = np.random.default_rng(23)
+    w = random_workload(rng, nx=6, ny=5, nv=nv, bc=inputs.BC_REFLECT, nspecies=2, fields_yee=1)
+    f0 = [(0.4 + 0.5 * s) * smooth_random_f(rng, w, s) for s in range(2)]
+    E = rng.standard_normal((3, w.ny_g, w.nx))
+    B = 2.0 * rng.standard_normal((3, w.ny_g, w.nx))
+    for s in range(2):
+        w.species[s].f_inf = 0.0 if s == 0 else -1.0
+    fg = [dev(f) for f in f0]
+    ctx = gpu.context_for(w, fg)
+    ctx.vlasov_step(0.07, dev(E), dev(B), gpu.STAGE_ALL)
+    assert ctx.check_code() == 0
+    for s in range(2):
+        w.species[s].f_inf = float(f0[s].max())
+        assert abs(w.species[s].f_inf - (0.4 + 0.5 * s)) < 1e-15
+        fo = f0[s].copy()
+        err, _ = orc.step(fo, osp(orc, w.species[s]), w.nx, w.ny, 0, w.lx, w.ly, 0.07, E, B, fields_yee=1, bc_lo=w.bc_y_lo,
+                          bc_hi=w.bc_y_hi, want_moments=False)
+        assert err == 0
+        got = fg[s].cpu().numpy()
+        assert rel_l2(got, fo) <= TOL1
+        assert np.abs(got - fo).max() <= 2e-13
+        # and the bound matters here: the same step with a loose f_inf differs
+        w.species[s].f_inf = 10.0
+        fl = f0[s].copy()
+        orc.step(fl, osp(orc, w.species[s]), w.nx, w.ny, 0, w.lx, w.ly, 0.07, E, B, fields_yee=1, bc_lo=w.bc_y_lo,
+                 bc_hi=w.bc_y_hi, want_moments=False)
+        assert np.abs(fl - fo).max() > 1e-6
+    ctx.close()
+
+
 @pytest.mark.parametrize("nv", [(32, 32, 32), (16, 16, 16), (24, 24, 24)])
 def test_vxv_step_with_moments_fused_into_the_last_velocity_pass(gpu, orc, nv):
     """NEXT-1: the order of the paper's coupled cycle, v/2 - x,y - v/2, with the 10 moments
