@@ -168,6 +168,43 @@ __global__ void __launch_bounds__(128) sweep_space_kernel(SpaceParams P) {
     if (bad) atomicCAS(P.err, 0, VLASOV_ESHIFT);
 }
 
+// z sweep of a short periodic line held in registers (3D3V, nz = NZ, every |sigma_z| < 1 and no pair of v_z cells
+// straddling v_z = 0): a thread owns two neighbouring v_z cells of one spatial column (ix, iy) and all NZ slabs of them.
+// All 2 NZ values are loaded at once (NZ independent 16-byte loads in flight), in the direction of the flow -- eq. (47)
+// is eq. (46) on the mirrored line -- so position i of the window is slab i (sigma >= 0) or NZ-1-i (sigma < 0); the
+// wrap-around is a compile-time index.  The general kernel above spends a short line on its prefetch queue and the
+// run-time wrap (0.50 of the HBM peak on 8 slabs).
+template <int NZ>
+__global__ void __launch_bounds__(128) sweep_z_reg_kernel(SpaceParams P) {
+    const long chunk = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (chunk >= P.S / 2) return;
+    const long v = chunk * 2;
+    const long col = (long)blockIdx.y * P.S + v;
+    const double va = P.vmin + ((int)(v % P.nv2) + 0.5) * P.dv;
+    const double sa = va * P.dts / P.dxx, sb = (va + P.dv) * P.dts / P.dxx;
+    const bool pos = sa + sb >= 0.0;
+    const double ba = fabs(sa), bb = fabs(sb);
+    double qa[NZ], qb[NZ];
+#pragma unroll
+    for (int i = 0; i < NZ; ++i) {
+        const double2 t = __ldcs(reinterpret_cast<const double2*>(P.src + col + (long)(pos ? i : NZ - 1 - i) * P.slab));
+        qa[i] = t.x; qb[i] = t.y;
+    }
+    double Ga[NZ], Gb[NZ];          // flux out of position i (through its downstream face)
+#pragma unroll
+    for (int i = 0; i < NZ; ++i) {
+        const int im = (i + NZ - 1) % NZ, ip = (i + 1) % NZ;
+        Ga[i] = partial_flux(qa[im], qa[i], qa[ip], ba, P.finf, P.limiter);
+        Gb[i] = partial_flux(qb[im], qb[i], qb[ip], bb, P.finf, P.limiter);
+    }
+#pragma unroll
+    for (int i = 0; i < NZ; ++i) {
+        const int im = (i + NZ - 1) % NZ;
+        const double2 o = make_double2(qa[i] + (Ga[im] - Ga[i]), qb[i] + (Gb[im] - Gb[i]));      // eq. (38)
+        __stcs(reinterpret_cast<double2*>(P.dst + col + (long)(pos ? i : NZ - 1 - i) * P.slab), o);
+    }
+}
+
 static int launch_space(vlasov_ctx* c, const Species& s, const double* src, double* dst, double dts, int axis,
                         int row0 = 0, int nrows = -1) {
     const Geom& G = c->G;
@@ -199,7 +236,10 @@ static int launch_space(vlasov_ctx* c, const Species& s, const double* src, doub
         Launch L(c, K_SWEEP_Z);
         if (pack) {
             dim3 grid((unsigned)((s.nvtot / 2 + threads - 1) / threads), (unsigned)(G.nyg * G.nx));
-            sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
+            if (G.nz == 8) sweep_z_reg_kernel<8><<<grid, threads, 0, c->stream>>>(P);
+            else if (G.nz == 4) sweep_z_reg_kernel<4><<<grid, threads, 0, c->stream>>>(P);
+            else if (G.nz == 16) sweep_z_reg_kernel<16><<<grid, threads, 0, c->stream>>>(P);
+            else sweep_space_kernel<2, 4><<<grid, threads, 0, c->stream>>>(P);
         } else {
             dim3 grid((unsigned)((s.nvtot + threads - 1) / threads), (unsigned)(G.nyg * G.nx));
             sweep_space_kernel<1, 4><<<grid, threads, 0, c->stream>>>(P);

@@ -460,6 +460,7 @@ int launch_sweep_xy(vlasov_ctx* c, const Species& s, const double* src, double* 
         else
         if (v32 && G.nx == 128 && C == 8) { if (lim) launch_xy_t<4, 1, 128, 32, 8>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128, 32, 8>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (v32 && G.nx == 128 && C == 16) { if (lim) launch_xy_t<4, 1, 128>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 128>(tm, P, xfirst, grid, threads, smem, c->stream); }
+        else if (v32 && G.nx == 32 && C == 32) { if (lim) launch_xy_t<4, 1, 32, 32, 32>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 32, 32, 32>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (v32 && G.nx == 64 && C == 32) { if (lim) launch_xy_t<4, 1, 64>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 64>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else if (xb == 4) { if (lim) launch_xy_t<4, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<4, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }
         else { if (lim) launch_xy_t<1, 1, 0>(tm, P, xfirst, grid, threads, smem, c->stream); else launch_xy_t<1, 0, 0>(tm, P, xfirst, grid, threads, smem, c->stream); }

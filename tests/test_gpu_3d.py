@@ -56,11 +56,13 @@ def osp(orc, s):
 @pytest.mark.parametrize("order", [0, 1])
 @pytest.mark.parametrize("bc", [inputs.BC_PERIODIC, inputs.BC_REFLECT])
 @pytest.mark.parametrize("nx,ny,nz,nv,dt", [(9, 6, 5, (8, 8, 8), 0.07), (16, 5, 3, (16, 16, 16), 0.02), (13, 4, 4, (6, 8, 10), 0.23),
-                                            (7, 4, 3, (4, 6, 5), 0.07)])
+                                            (7, 4, 3, (4, 6, 5), 0.07), (6, 4, 8, (8, 8, 8), 0.02), (5, 3, 16, (4, 4, 8), 0.02),
+                                            (5, 3, 4, (4, 6, 8), 0.02)])
 def test_full_3d3v_step(gpu, orc, order, bc, nx, ny, nz, nv, dt):
     """x/2 y/2 z/2 - v - z/2 y/2 x/2 (and VXV) for two species with Yee fields.  (16,5,3,16^3): shifts below one cell, the
     fused x,y stage per z slab and the TMA velocity kernels (fused moments under VXV); dt = 0.23: multi-cell shifts in all
-    three directions with wrap-around, the general kernels; (4,6,5): an odd nv[2], one cell per thread."""
+    three directions with wrap-around, the general kernels; (4,6,5): an odd nv[2], one cell per thread; nz = 8, 16, 4 with dt = 0.02: the z sweep
+    that holds a whole periodic line in registers."""
     import torch
     rng = np.random.default_rng(51)
     w = workload3d(nx, ny, nz, nv, bc, nspecies=2)
