@@ -118,12 +118,14 @@ int launch_moments(vlasov_ctx* c, const Species& s, const double* f, double* out
         const int nchunk = s.nv[1] * s.nv[2] / (s.nv[2] % 2 == 0 ? 2 : 1);
         auto waste = [&](int t) { return ((nchunk + t - 1) / t) * t - nchunk; };
         int nt = MOM_THREADS;
+        if (waste(192) == 0 && waste(nt) > 0) nt = 192;      // 48^3: 1152 pairs of columns = 6 x 192 (1.19 -> 1.12 ms)
         if (nchunk < 2 * MOM_THREADS) {
             if (waste(128) < waste(nt)) nt = 128;
             if (waste(96) < waste(nt)) nt = 96;
         }
         if (s.nv[2] % 2 == 0) {
-            if (nt == 128) moments_kernel<2, 128><<<P.ncell_out, 128, 0, c->stream>>>(P);
+            if (nt == 192) moments_kernel<2, 192><<<P.ncell_out, 192, 0, c->stream>>>(P);
+            else if (nt == 128) moments_kernel<2, 128><<<P.ncell_out, 128, 0, c->stream>>>(P);
             else if (nt == 96) moments_kernel<2, 96><<<P.ncell_out, 96, 0, c->stream>>>(P);
             else moments_kernel<2><<<P.ncell_out, MOM_THREADS, 0, c->stream>>>(P);
         } else {
