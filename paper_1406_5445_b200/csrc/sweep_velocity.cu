@@ -679,14 +679,51 @@ __global__ void __launch_bounds__(V_THREADS, 3) vsweep_yz_kernel(VParams P) {
 __host__ __device__ constexpr int yz_tma_planes(int cn) { return cn == 40 ? VL_YZ40_PLANES : cn == 32 ? VL_YZ32_PLANES : 2048 / (cn * cn) > 0 ? 2048 / (cn * cn) : 1; }
 __host__ __device__ constexpr int yz_tma_threads(int cn) { return (yz_tma_planes(cn) * cn * ((cn + 7) / 8) + 31) / 32 * 32; }
 static_assert(yz_tma_threads(16) == 256 && yz_tma_threads(24) == 224 && yz_tma_threads(48) == 288, "");
-// resident CTAs per SM the kernel is compiled for: 3 (80 registers at 256 threads); one 48x48 plane has 288 work items
-// (9 warps) and 69 KB of shared memory: 2 CTAs per SM
-__host__ __device__ constexpr int yz_tma_minb(int cn) { return cn == 48 || (cn == 40 && VL_YZ40_PLANES > 1) ? 2 : cn == 32 && VL_YZ32_PLANES == 1 ? 6 : cn == 32 && VL_YZ32_PLANES == 4 ? 1 : VL_YZ_MINB; }
+// resident CTAs per SM the kernel is compiled for: 3 (80 registers at 256 threads; 70 at the 288 threads of a 48x48 plane)
+// 48x48: 288 threads and 69 KB per CTA; 3 CTAs per SM (27 warps at 70 registers, no spills) measured 12 % faster than 2
+// (18 warps): nv48 6.89 -> 6.08 ms per cycle.  40x40 with one plane per tile and 4 CTAs (28 warps) measured slower than two
+// planes and 2 CTAs (26 warps): 7.92 -> 8.20 ms.
+#ifndef VL_YZ48_MINB
+#define VL_YZ48_MINB 3
+#endif
+#ifndef VL_YZ40_MINB
+#define VL_YZ40_MINB (VL_YZ40_PLANES > 1 ? 2 : VL_YZ_MINB)
+#endif
+// 32x32: the compact layout leaves room for 4 CTAs per SM (57 KB each), and the kernel fits 62 registers without spills,
+// but 32 warps at 62 registers measured no faster than 24 at 80 (2.87 against 2.84 ms per cycle of config 3): 3.
+// 24x24: 4 CTAs (28 warps at 69 registers) against 3 (21 warps): nv24 0.803 -> 0.718 ms.
+#ifndef VL_YZ32_MINB
+#define VL_YZ32_MINB (VL_YZ32_PLANES == 1 ? 6 : VL_YZ32_PLANES == 4 ? 1 : 3)
+#endif
+#ifndef VL_YZ24_MINB
+#define VL_YZ24_MINB 4
+#endif
+__host__ __device__ constexpr int yz_tma_minb(int cn) { return cn == 48 ? VL_YZ48_MINB : cn == 40 ? VL_YZ40_MINB : cn == 32 ? VL_YZ32_MINB : cn == 24 ? VL_YZ24_MINB : VL_YZ_MINB; }
 
 // MOM = 1 (VXV order): the 10 raw velocity moments, eqs. (2)-(4), of the final f are
 // reduced in this kernel.  A CTA then takes WHOLE spatial cells (all tiles of a cell one after the other), sums its
 // cells while it stores them, and writes the moments of the cell itself: no partial sums in global memory, no
 // atomics, a fixed summation order.  For planes where a thread keeps its i_vz over a tile (16x16, 32x32).
+// Shared-memory layout of the TMA-staged kernel, in doubles.  Staging: pad rows of zeros around every plane (>= V_PAD;
+// every TMA box must start 128-byte aligned: 8 rows of any even N2 do, and any number of rows when a row is a multiple
+// of 128 bytes).  Bf (between the sweeps): rows of N2 + V_PAD, zero pads.  A (output): written by the vz sweep and read
+// by the store loop only, so it needs no pads, just an odd pitch (lanes of the vz sweep run along y).
+#ifndef VL_YZ_COMPACT
+#define VL_YZ_COMPACT 1
+#endif
+__host__ __device__ constexpr int yz_tma_spad(int cn) { return VL_YZ_COMPACT && cn % 16 == 0 ? V_PAD : 8; }
+// (the walks may look at the 4th row before a line, whatever it holds: one more row before the first plane)
+__host__ __device__ constexpr int yz_tma_spad0(int cn) { return yz_tma_spad(cn) > V_PAD ? yz_tma_spad(cn) : V_PAD + 1; }
+__host__ __device__ constexpr int yz_tma_stg(int cn) { return ((yz_tma_spad0(cn) + yz_tma_planes(cn) * (cn + yz_tma_spad(cn))) * cn + 15) & ~15; }
+__host__ __device__ constexpr int yz_tma_buf(int cn) { return (V_PAD * (cn + V_PAD) + V_PAD + yz_tma_planes(cn) * (cn + V_PAD) * (cn + V_PAD) + 1) & ~1; }
+__host__ __device__ constexpr int yz_tma_rsa(int cn) { return VL_YZ_COMPACT ? (cn | 1) : cn + V_PAD; }
+__host__ __device__ constexpr int yz_tma_psa(int cn) { return VL_YZ_COMPACT ? cn * yz_tma_rsa(cn) : (cn + V_PAD) * (cn + V_PAD); }
+__host__ __device__ constexpr int yz_tma_offa(int cn) { return VL_YZ_COMPACT ? 0 : V_PAD * (cn + V_PAD) + V_PAD; }
+__host__ __device__ constexpr int yz_tma_bufa(int cn) { return (yz_tma_offa(cn) + yz_tma_planes(cn) * yz_tma_psa(cn) + 1) & ~1; }
+__host__ __device__ constexpr size_t yz_tma_smem(int cn) {
+    return (size_t)(yz_tma_stg(cn) + yz_tma_buf(cn) + yz_tma_bufa(cn)) * 8 + 16 + TAB * 8 + 8 * 10 * 8;
+}
+
 template <int LIM, int CN, int MOM = 0>
 __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
     extern __shared__ __align__(128) double sm[];
@@ -695,10 +732,13 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
     constexpr int nseg = (CN + 7) / 8, seglen = (CN + nseg - 1) / nseg;
     constexpr int RS = N2 + V_PAD, PS = (N1 + V_PAD) * RS, OFF = V_PAD * RS + V_PAD;
     constexpr int BUF = (OFF + ct * PS + 1) & ~1;
-    constexpr int SPAD = 8;                                      // pad rows of the staging buffer: >= V_PAD, and 8 rows of
+    constexpr int SPAD = yz_tma_spad(CN);                        // pad rows of the staging buffer: >= V_PAD, and 8 rows of
                                                                  // any even N2 keep every TMA box 128-byte aligned
-    constexpr int SROWS = SPAD + ct * (N1 + SPAD);               // staging rows of N2 doubles
+    constexpr int SP0 = yz_tma_spad0(CN);                        // rows before the first plane
+    constexpr int SROWS = SP0 + ct * (N1 + SPAD);                // staging rows of N2 doubles
     constexpr int STG = (SROWS * N2 + 15) & ~15;                 // keeps Bf 128-byte aligned
+    static_assert(STG == yz_tma_stg(CN) && BUF == yz_tma_buf(CN), "layout helpers");
+    constexpr int RSA = yz_tma_rsa(CN), PSA = yz_tma_psa(CN), OFFA = yz_tma_offa(CN), BUFA = yz_tma_bufa(CN);      // output buffer A
     // The work items of a sweep (ct CN nseg) need not fill the last warp.  Its idle lanes REPEAT the items of the 32
     // lanes before them (same reads, same values written to the same places), so that every warp that works at all is
     // whole: the walks vote with the full mask, no __activemask() bookkeeping, no divergence guards around the votes.
@@ -710,17 +750,17 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
     double* St = sm;
     double* Bf = sm + STG;
     double* A = Bf + BUF;
-    const unsigned bar = smem_addr(A + BUF);
-    const double* tab = A + BUF + 2;               // the tile's sweep-table row rides along with the tile (16-byte aligned)
-    double* red = A + BUF + 2 + TAB;               // MOM: [warps][10] partial sums of a spatial cell
+    const unsigned bar = smem_addr(A + BUFA);
+    const double* tab = A + BUFA + 2;               // the tile's sweep-table row rides along with the tile (16-byte aligned)
+    double* red = A + BUFA + 2 + TAB;               // MOM: [warps][10] partial sums of a spatial cell
     static_assert((TAB * 8) % 16 == 0, "bulk copy size");
     // zero: the staging pad rows (never written again), Bf and A entirely (their cells are overwritten per tile)
+    for (int e = threadIdx.x; e < SP0 * N2; e += NT) St[e] = 0.0;
     for (int e = threadIdx.x; e < SPAD * N2; e += NT) {
-        St[e] = 0.0;
 #pragma unroll
-        for (int p = 0; p < ct; ++p) St[(SPAD + p * (N1 + SPAD) + N1) * N2 + e] = 0.0;
+        for (int p = 0; p < ct; ++p) St[(SP0 + p * (N1 + SPAD) + N1) * N2 + e] = 0.0;
     }
-    for (int e = threadIdx.x; e < 2 * BUF; e += NT) Bf[e] = 0.0;
+    for (int e = threadIdx.x; e < BUF + BUFA; e += NT) Bf[e] = 0.0;
     if (threadIdx.x == 0) mbar_init(bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
@@ -730,7 +770,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
         bulk_g2s(smem_addr(tab), P.table + (long)cell * TAB, TAB * 8, bar);
 #pragma unroll
         for (int p = 0; p < ct; ++p)
-            tma_g2s_2d(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2) * 8, &tmap, 0, (cell * P.nv0 + p0 + p) * N1, bar);
+            tma_g2s_2d(sSt + (unsigned)((SP0 + p * (N1 + SPAD)) * N2) * 8, &tmap, 0, (cell * P.nv0 + p0 + p) * N1, bar);
     };
     // (spatial cell, tile within the cell) of this CTA's tiles, advanced without a division per tile.  MOM: the CTA
     // owns the cells blockIdx.x, blockIdx.x + gridDim.x, ... and walks the tiles of a cell in order.
@@ -742,9 +782,9 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
     // staging map of the store loop (as in the plain kernel)
     const int z_init = threadIdx.x % N2, row_init = threadIdx.x / N2;
     const int y_init = row_init % N1;
-    const unsigned so_init = OFF + (row_init / N1) * PS + y_init * RS + z_init;
+    const unsigned so_init = OFFA + (row_init / N1) * PSA + y_init * RSA + z_init;
     constexpr int dz = NT % N2, drow = NT / N2, dy = drow % N1;
-    constexpr unsigned dso = dz + dy * RS + (drow / N1) * PS;
+    constexpr unsigned dso = dz + dy * RSA + (drow / N1) * PSA;
     constexpr int ncellt = ct * plane;
     double T0 = 0.0, Tx = 0.0, Txx = 0.0, Ty = 0.0, Tyy = 0.0, Txy = 0.0;      // MOM: this thread's sums over a spatial cell
     int it = 0;
@@ -770,7 +810,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
                 const int a = seg * seglen, b = a + seglen;          // CN is a multiple of 8: whole segments
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM, FW, 1, VL_YZ_BATCH>(sSt + (unsigned)((SPAD + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH>(sSt + (unsigned)((SP0 + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
@@ -784,7 +824,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 const int p = l / N1, y = l - p * N1;
                 const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
                 const int a = seg * seglen, b = a + seglen;
-                OutShared o{smem_addr(A + OFF + p * PS + y * RS + a), 8};
+                OutShared o{smem_addr(A + OFFA + p * PSA + y * RSA + a), 8};
                 march_cells<LIM, FW, 1, VL_YZ_BATCH>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
             }
         }
@@ -800,7 +840,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 double r0 = 0.0, r1 = 0.0, r2 = 0.0;
 #pragma unroll
                 for (int j = 0; j < EPP; ++j) {
-                    const double fv = lds(sA + (so_init + pp * PS + j * drow * RS) * 8);
+                    const double fv = lds(sA + (so_init + pp * PSA + j * drow * RSA) * 8);
                     __stcs(fb + threadIdx.x + (pp * EPP + j) * NT, fv);
                     const double vy = vy0 + (j * drow) * P.dv[1];
                     const double t = vy * fv;
@@ -842,8 +882,8 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 for (int e = threadIdx.x; e < ncellt; e += NT) {
                     __stcs(fb + e, lds(sA + so * 8));
                     z += dz; y += dy; so += dso;
-                    if (z >= N2) { z -= N2; so += RS - N2; ++y; }
-                    if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+                    if (z >= N2) { z -= N2; so += RSA - N2; ++y; }
+                    if (y >= N1) { y -= N1; so += PSA - N1 * RSA; }
                 }
             } else {
 #pragma unroll 4
@@ -851,8 +891,8 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                     const int e = threadIdx.x + i * NT;
                     if (e < ncellt) __stcs(fb + e, lds(sA + so * 8));
                     z += dz; y += dy; so += dso;
-                    if (z >= N2) { z -= N2; so += RS - N2; ++y; }
-                    if (y >= N1) { y -= N1; so += PS - N1 * RS; }
+                    if (z >= N2) { z -= N2; so += RSA - N2; ++y; }
+                    if (y >= N1) { y -= N1; so += PSA - N1 * RSA; }
                 }
             }
         }
@@ -977,9 +1017,7 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (spec == 24) kt = lim ? vsweep_yz_tma_kernel<1, 24> : vsweep_yz_tma_kernel<0, 24>;
             if (spec == 40) kt = lim ? vsweep_yz_tma_kernel<1, 40> : vsweep_yz_tma_kernel<0, 40>;
             if (spec == 48) kt = lim ? vsweep_yz_tma_kernel<1, 48> : vsweep_yz_tma_kernel<0, 48>;
-            const size_t srows = 8 + (size_t)pt * (s.nv[1] + 8);
-            const size_t stg = (srows * s.nv[2] + 15) & ~(size_t)15;
-            const size_t smem_t = (stg + 2 * buf) * 8 + 16 + TAB * 8 + 8 * 10 * 8;
+            const size_t smem_t = yz_tma_smem(spec);
             // moments of the final f reduced in the same pass (VXV order): CTAs take whole spatial cells
             const bool mom = mom_out && !ghost && (spec == 16 || spec == 32);
             if (mom) {
