@@ -500,16 +500,24 @@ __global__ void __launch_bounds__(V_THREADS, CN ? 3 : 4) vsweep_x_kernel(VParams
 // another cell and are scaled).  Shared memory, in rows of 128 doubles:
 //   [V_PAD zero rows][CN rows, buffer 0][V_PAD zero rows][CN rows, buffer 1][V_PAD zero rows][2 mbarriers]
 // ------------------------------------------------------------------------------------------------
+// Threads of a CTA of the TMA-fed vx kernel: a tile has 128 (CN / 8) work items (8-cell segments of 128 columns).  24^3:
+// 384 items on 192 threads, 3 CTAs per SM, instead of one and a half trips of 256 threads: nv24 0.336 -> 0.307 ms per
+// cycle.  40^3 (640 items) stays at 256 threads: 320 threads at the 102 registers that leaves measured slower (3.21 ->
+// 3.52 ms per cycle of config 4).
+__host__ __device__ constexpr int x_tma_threads(int cn) { return cn == 24 ? 192 : V_THREADS; }
+__host__ __device__ constexpr int x_tma_minb(int cn) { return cn == 24 ? 3 : 2; }
+
 template <int LIM, int CN>
-__global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
+__global__ void __launch_bounds__(x_tma_threads(CN), x_tma_minb(CN)) vsweep_x_tma_kernel(const __grid_constant__ CUtensorMap tmap, VParams P) {
     extern __shared__ __align__(128) double sm[];
     // the last tile of a plane may be ragged (24^2, 40^2: 64 columns; the box is zero-filled past the plane): a
     // multiple of 32, so warps stay whole
     constexpr int CT = 128, N = CN, plane = CN * CN, ntile = (plane + CT - 1) / CT, nsegx = CN / 8, seglen = 8;
     constexpr int ROWS = 3 * V_PAD + 2 * CN;
+    constexpr int NT = x_tma_threads(CN);
     static_assert(plane % 32 == 0 && CN % 8 == 0, "whole warps, whole segments");
     // only the three pad strips are ever written by threads (zeros, once); the buffers belong to the TMA unit
-    for (int e = threadIdx.x; e < V_PAD * CT; e += V_THREADS) {
+    for (int e = threadIdx.x; e < V_PAD * CT; e += NT) {
         sm[e] = 0.0; sm[(V_PAD + CN) * CT + e] = 0.0; sm[(2 * V_PAD + 2 * CN) * CT + e] = 0.0;
     }
     const unsigned bar0 = smem_addr(sm + ROWS * CT);
@@ -538,7 +546,7 @@ __global__ void __launch_bounds__(V_THREADS, 2) vsweep_x_tma_kernel(const __grid
         const double* A = sm + (V_PAD + b * (CN + V_PAD)) * CT;
         mbar_wait(bar0 + 8 * b, (it >> 1) & 1);
 #pragma unroll
-        for (int wi = threadIdx.x; wi < CT * nsegx; wi += V_THREADS) {
+        for (int wi = threadIdx.x; wi < CT * nsegx; wi += NT) {
             const int seg = wi / CT, c = wi - seg * CT;
             const int col = c0 + c;
             if (plane % CT != 0 && col >= plane) continue;
@@ -967,9 +975,10 @@ int launch_vsweeps(vlasov_ctx* c, const Species& s, double* f, int row0, int nro
             if (tspec == 40) kt = lim ? vsweep_x_tma_kernel<1, 40> : vsweep_x_tma_kernel<0, 40>;
             if (tspec == 48) kt = lim ? vsweep_x_tma_kernel<1, 48> : vsweep_x_tma_kernel<0, 48>;
             const size_t smem_t = (size_t)(3 * V_PAD + 2 * tspec) * 128 * 8 + 16;
-            const int grid = min(P.ntot, resident_ctas(kt, smem_t));
+            const int ntx = x_tma_threads(tspec);
+            const int grid = min(P.ntot, resident_ctas(kt, smem_t, ntx));
             Launch L(c, K_VSWEEP_X);
-            kt<<<grid, V_THREADS, smem_t, c->stream>>>(tm, P);
+            kt<<<grid, ntx, smem_t, c->stream>>>(tm, P);
         } else {
             const int grid = min(P.ntot, resident_ctas(k, smem));
             Launch L(c, K_VSWEEP_X);
