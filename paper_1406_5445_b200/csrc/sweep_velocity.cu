@@ -124,6 +124,21 @@ int launch_lorentz_table(vlasov_ctx* c, const Species& s, const double* E, const
     return cudaGetLastError() == cudaSuccess ? VLASOV_OK : VLASOV_ECUDA;
 }
 
+// The two weights of eq. (46) as functions of alpha = b: c1 = (1-b)(2-b)/6, c2 = (1-b)(1+b)/6.  Written so that no
+// instruction has more than one constant operand (1 and 1/2 are immediates, 1/6 comes from the constant bank): with two,
+// one of them has to be moved into registers again at every face (8 of the ~50 instructions of a face were such moves).
+//   c2 = (1 - b^2) / 6,   c1 + c2 = (1 - b) / 2.
+__device__ __forceinline__ void pfc_weights(double b, double& c1, double& c2) {
+#ifdef VL_POLY_OLD
+    const double b2 = b * b;
+    c1 = fma(b2, 1.0 / 6.0, fma(b, -0.5, 1.0 / 3.0));
+    c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+#else
+    c2 = (1.0 - b * b) * (1.0 / 6.0);
+    c1 = fma(1.0 - b, 0.5, -c2);
+#endif
+}
+
 // Flux through face k (between cells k-1 and k, 1 <= k <= N-1) of a ZERO-PADDED line in shared memory:
 // L = shared byte address of cell 0, st8 = stride in bytes, cells -3..-1 and N..N+2 hold zeros (f = 0
 // outside the box, R7).  eq. (46) for sigma >= 0, eq. (47) (sum repaired, R5) for sigma < 0: the same
@@ -155,9 +170,8 @@ __device__ __forceinline__ double face_flux_pad(unsigned L, int st8, int N, int 
     double sp, sm;
     slopes_fast<LIM>(fm, f0, fp, finf, sp, sm);
     // alpha [ f0 + (1-a)(2-a)/6 sp + (1-a)(1+a)/6 sm ]: the two weights as polynomials in alpha
-    const double b2 = b * b;
-    const double c1 = fma(b2, 1.0 / 6.0, fma(b, -0.5, 1.0 / 3.0));
-    const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+    double c1, c2;
+    pfc_weights(b, c1, c2);
     const double phi = fma(b, fma(c1, sp, fma(c2, sm, f0)), sum);
     // phi for sigma >= 0, -phi otherwise: flip the sign bit with sigma's
     return __hiloint2double(__double2hiint(phi) ^ (sg & 0x80000000), __double2loint(phi));
@@ -222,9 +236,8 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
             double sp, sm;
             slopes_fast<LIM, FULL>(q[m], q[m + 1], q[m + 2], finf, sp, sm);
             const double bq = fabs(sig);
-            const double b2 = bq * bq;
-            const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
-            const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+            double c1, c2;
+            pfc_weights(bq, c1, c2);
             double G = bq * fma(c1, sp, fma(c2, sm, q[m + 1]));
             if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
             if (m > 0) out.put(q[m + 1] + (Gp - G));     // eq. (38) for the cell between walk faces m-1 and m
@@ -284,9 +297,8 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
             const int m = m0 + i;
             if (m > SEG) break;
             const double bq = fabs(sig);
-            const double b2 = bq * bq;
-            const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
-            const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+            double c1, c2;
+            pfc_weights(bq, c1, c2);
             double G = bq * fma(c1, sp[i], fma(c2, sm[i], q[m + 1]));
             if ((m == 0 && zero_first) || (m == SEG && zero_last)) G = 0.0;
             if (m > 0) out.put(q[m + 1] + (Gp - G));     // eq. (38) for the cell between walk faces m-1 and m
@@ -342,9 +354,8 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
         const double f0 = lds(F), fm = lds(F - uu), fp = lds(F + uu);
         double sp, sm;
         slopes_fast<LIM, FULL>(fm, f0, fp, finf, sp, sm);
-        const double b2 = bq * bq;
-        const double c1 = fma(b2, 1.0 / 6.0, fma(bq, -0.5, 1.0 / 3.0));
-        const double c2 = fma(b2, -1.0 / 6.0, 1.0 / 6.0);
+        double c1, c2;
+        pfc_weights(bq, c1, c2);
         double G = bs * fma(c1, sp, fma(c2, sm, f0));
         if (m == 0) {
             if (zero_first) G = 0.0;
