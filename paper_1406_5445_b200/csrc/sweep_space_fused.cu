@@ -70,7 +70,8 @@ __device__ __forceinline__ int hi_abs(double d) { return __double2hiint(d) & 0x7
 // N partial fluxes alpha [ f0 + c1 eps+ d+ + c2 eps- d- ] of the cells q[1..N] of a line piece q[0..N+1]
 // (q ordered in the direction of the flow, so eq. (47) is the same call on the reversed piece).
 // The limiter test is batched: one vote per call, and the usual answer is "nobody".
-template <int N, int LIM>
+// FULL: every lane of the warp makes this call together (the CTA-uniform copies of the row loop): votes with the full mask.
+template <int N, int LIM, int FULL = 0>
 __device__ __forceinline__ void flux_line(const double (&q)[N + 2], const Weights& W, double finf, double (&G)[N]) {
     double d[N + 1];
 #pragma unroll
@@ -82,11 +83,11 @@ __device__ __forceinline__ void flux_line(const double (&q)[N + 2], const Weight
             if (i < N) { hmin = min(hmin, __double2hiint(q[i + 1])); hmax = max(hmax, __double2hiint(q[i + 1])); }
             dmax = max(dmax, hi_abs(d[i]));
         }
-        if (__any_sync(__activemask(), batch_may_need(hmin, hmax, dmax, finf))) {
+        if (__any_sync(FULL ? 0xffffffffu : __activemask(), batch_may_need(hmin, hmax, dmax, finf))) {
 #pragma unroll
             for (int i = 0; i < N; ++i) {
                 double sp, sm;
-                slopes_fast<1>(q[i], q[i + 1], q[i + 2], finf, sp, sm);
+                slopes_fast<1, FULL>(q[i], q[i + 1], q[i + 2], finf, sp, sm);
                 G[i] = fma(W.w2, sm, fma(W.w1, sp, W.w0 * q[i + 1]));
             }
             return;
@@ -100,7 +101,7 @@ __device__ __forceinline__ void flux_line(const double (&q)[N + 2], const Weight
 // sbuf ([x][c], this thread's column at byte offset cofs).  DIR = +1: sigma >= 0, eq. (46); DIR = -1: eq. (47),
 // the same on the mirrored line.  val[i] = new average, eq. (38), of owned cell item(k, i); the flux through
 // the chunk border is carried over (same arithmetic on the same inputs: identical value).
-template <int XB, int CH, int LIM, int DIR>
+template <int XB, int CH, int LIM, int DIR, int FULL = 0>
 __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH], unsigned sbuf, int ix0, int nx, int C8,
                                         unsigned cofs, const Weights& W, double finf) {
     // position p = 0 .. XB+2 along the flow: cell ix0-2+p (DIR > 0) or ix0+XB+1-p (DIR < 0)
@@ -112,7 +113,7 @@ __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH],
         if (p < 2 || p == XB + 2) { if (ix < 0) ix += nx; else if (ix >= nx) ix -= nx; }
         q[i] = lds(sbuf + ix * C8 + cofs);
     }
-    flux_line<CH + 1, LIM>(q, W, finf, G);         // fluxes out of positions 1+k CH .. 1+k CH+CH
+    flux_line<CH + 1, LIM, FULL>(q, W, finf, G);         // fluxes out of positions 1+k CH .. 1+k CH+CH
     if (k > 0) G[0] = carry;
     carry = G[CH];
 #pragma unroll
@@ -136,12 +137,13 @@ __device__ __forceinline__ void y_batch(const double (&ya)[NB], const double (&y
         dlo[i] = yb[i] - ya[i]; dhi[i] = gx[i] - yb[i];
         if (LIM) { hmin = min(hmin, __double2hiint(yb[i])); hmax = max(hmax, __double2hiint(yb[i])); dup = max(dup, hi_abs(dhi[i])); }
     }
-    const bool slow = LIM && __any_sync(__activemask(), batch_may_need(hmin, hmax, max(dup, ydmax), finf));
+    constexpr int FULL = YD != 0 ? 1 : 0;          // a known direction means a CTA-uniform copy of the row loop: whole warps
+    const bool slow = LIM && __any_sync(FULL ? 0xffffffffu : __activemask(), batch_may_need(hmin, hmax, max(dup, ydmax), finf));
     ydmax = dup;
 #pragma unroll
     for (int i = 0; i < NB; ++i) {
         double sp = ypos ? dhi[i] : -dlo[i], sm = ypos ? dlo[i] : -dhi[i];
-        if (slow) { if (ypos) slopes_fast<1>(ya[i], yb[i], gx[i], finf, sp, sm); else slopes_fast<1>(gx[i], yb[i], ya[i], finf, sp, sm); }
+        if (slow) { if (ypos) slopes_fast<1, FULL>(ya[i], yb[i], gx[i], finf, sp, sm); else slopes_fast<1, FULL>(gx[i], yb[i], ya[i], finf, sp, sm); }
         const double Gn = fma(Wy.w2, sm, fma(Wy.w1, sp, Wy.w0 * yb[i]));
         h[i] = ypos ? yb[i] + (yG[i] - Gn) : ya[i] + (Gn - yG[i]);
         yG[i] = Gn;
@@ -279,7 +281,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
             for (int k = 0; k < XB / CH; ++k) {
                 double gx[CH];
                 if (XD > 0 || (XD == 0 && Wx.pos)) {
-                    x_chunk<XB, CH, LIM, 1>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, 1, (XD != 0)>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
                     double ya[CH], yb[CH], g[CH], h[CH];
 #pragma unroll
                     for (int i = 0; i < CH; ++i) { const int it = k * CH + i; ya[i] = PAR == 0 ? A[it] : B[it]; yb[i] = PAR == 0 ? B[it] : A[it]; g[i] = yG[it]; }
@@ -292,7 +294,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
                         if (store) __stcs(po + (long)it * S, h[i]);
                     }
                 } else {
-                    x_chunk<XB, CH, LIM, -1>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, -1, (XD != 0)>(k, carry, gx, sraw, ix0, nx, X8, cofs, Wx, finf);
                     double ya[CH], yb[CH], g[CH], h[CH];
 #pragma unroll
                     for (int i = 0; i < CH; ++i) { const int it = XB - 1 - (k * CH + i); ya[i] = PAR == 0 ? A[it] : B[it]; yb[i] = PAR == 0 ? B[it] : A[it]; g[i] = yG[it]; }
@@ -327,13 +329,13 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
             for (int k = 0; k < XB / CH; ++k) {
                 double o[CH];
                 if (XD > 0 || (XD == 0 && Wx.pos)) {
-                    x_chunk<XB, CH, LIM, 1>(k, carry, o, sh, ix0, nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, 1, (XD != 0)>(k, carry, o, sh, ix0, nx, X8, cofs, Wx, finf);
                     if (store) {
 #pragma unroll
                         for (int i = 0; i < CH; ++i) __stcs(po + (long)(k * CH + i) * S, o[i]);
                     }
                 } else {
-                    x_chunk<XB, CH, LIM, -1>(k, carry, o, sh, ix0, nx, X8, cofs, Wx, finf);
+                    x_chunk<XB, CH, LIM, -1, (XD != 0)>(k, carry, o, sh, ix0, nx, X8, cofs, Wx, finf);
                     if (store) {
 #pragma unroll
                         for (int i = 0; i < CH; ++i) __stcs(po + (long)(XB - 1 - (k * CH + i)) * S, o[i]);
