@@ -262,11 +262,30 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
 
     // one row; PAR = parity of r + 2: rows (r-2, r-1) = (A, B) if PAR == 0 else (B, A); the new row replaces r-2
     // XD, YD: the flow directions as compile-time constants (+1 / -1) where the whole CTA shares them, 0: per thread
+#ifndef VL_XY_WREG
+#define VL_XY_WREG 1
+#endif
+    double rw[6];
+    {
+        Weights W0x, W0y;
+        W0x.set((P.vminx + (ivx + 0.5) * P.dvx) * P.kx);
+        W0y.set((P.vminy + (ivy + 0.5) * P.dvy) * P.ky);
+        rw[0] = W0x.w0; rw[1] = W0x.w1; rw[2] = W0x.w2; rw[3] = W0y.w0; rw[4] = W0y.w1; rw[5] = W0y.w2;
+    }
     auto row = [&](auto par, auto xd, auto yd, int r, int stage, unsigned phase) {
         constexpr int PAR = decltype(par)::value, XD = decltype(xd)::value, YD = decltype(yd)::value;
         Weights Wx, Wy;
-        Wx.w0 = wt[0 * C + c]; Wx.w1 = wt[1 * C + c]; Wx.w2 = wt[2 * C + c]; Wx.pos = XD == 0 ? xpos : XD > 0;
-        Wy.w0 = wt[3 * C + c]; Wy.w1 = wt[4 * C + c]; Wy.w2 = wt[5 * C + c]; Wy.pos = YD == 0 ? ypos : YD > 0;
+#if VL_XY_WREG
+        if (XD != 0) {       // the CTA-uniform copies have the registers to keep the six weights (98 of 128)
+            Wx.w0 = rw[0]; Wx.w1 = rw[1]; Wx.w2 = rw[2]; Wy.w0 = rw[3]; Wy.w1 = rw[4]; Wy.w2 = rw[5];
+        } else
+#endif
+        {
+            Wx.w0 = wt[0 * C + c]; Wx.w1 = wt[1 * C + c]; Wx.w2 = wt[2 * C + c];
+            Wy.w0 = wt[3 * C + c]; Wy.w1 = wt[4 * C + c]; Wy.w2 = wt[5 * C + c];
+        }
+        Wx.pos = XD == 0 ? xpos : XD > 0;
+        Wy.pos = YD == 0 ? ypos : YD > 0;
         const unsigned sraw = raw0 + stage * rowbytes;
         mbar_wait(bar0 + 8 * stage, phase);
         const int orow = r - orow_shift;
