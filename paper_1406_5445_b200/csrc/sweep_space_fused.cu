@@ -120,6 +120,27 @@ __device__ __forceinline__ void x_chunk(int k, double& carry, double (&val)[CH],
     for (int i = 0; i < CH; ++i) val[i] = q[i + 2] + (G[i] - G[i + 1]);
 }
 
+// x_chunk for a whole x block (CH = XB) whose own cells the thread still holds in registers (own[i] = cell ix0 + i, the
+// y-swept values it has just written to the shared row): only the three halo cells are read from shared memory.
+template <int XB, int LIM, int DIR, int FULL>
+__device__ __forceinline__ void x_chunk_own(const double (&own)[XB], double (&val)[XB], unsigned sbuf, int ix0, int nx, int C8,
+                                            unsigned cofs, const Weights& W, double finf) {
+    double q[XB + 3], G[XB + 1];
+#pragma unroll
+    for (int p = 0; p < XB + 3; ++p) {
+        if (p >= 2 && p < XB + 2) {
+            q[p] = own[DIR > 0 ? p - 2 : XB + 1 - p];
+        } else {
+            int ix = DIR > 0 ? ix0 - 2 + p : ix0 + XB + 1 - p;
+            if (ix < 0) ix += nx; else if (ix >= nx) ix -= nx;
+            q[p] = lds(sbuf + ix * C8 + cofs);
+        }
+    }
+    flux_line<XB + 1, LIM, FULL>(q, W, finf, G);
+#pragma unroll
+    for (int i = 0; i < XB; ++i) val[i] = q[i + 2] + (G[i] - G[i + 1]);
+}
+
 // NB steps of the y march at once (the owned cells of one x chunk): rows (r-2, r-1, r) = (ya, yb, gx) -> new average
 // h of row r-1 (sigma_y >= 0, eq. 46) or r-2 (sigma_y < 0, eq. 47 on the mirrored line).  One limiter vote for all
 // NB of them, so that the flux evaluations are independent instruction streams.
@@ -185,6 +206,9 @@ template <int XB, int LIM, int XFIRST, int SP, int NV = 32, int KC = xy_default_
 #endif
 #ifndef VL_XY_UNIDIR
 #define VL_XY_UNIDIR 1
+#endif
+#ifndef VL_XY_OWN
+#define VL_XY_OWN 1
 #endif
 __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const __grid_constant__ CUtensorMap tmap, XYParams P) {
     extern __shared__ __align__(128) unsigned char smraw[];
@@ -330,8 +354,9 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
             __syncthreads();                       // everybody is done reading raw row r
         } else {
             const unsigned sh = hb0 + (unsigned)PAR * rowbytes;
+            double h[XB];
             {
-                double gx[XB], h[XB];
+                double gx[XB];
 #pragma unroll
                 for (int i = 0; i < XB; ++i) gx[i] = lds(sraw + own + i * X8);
                 if (PAR == 0) y_batch<XB, LIM, YD>(A, B, yG, gx, Wy, finf, h, ydm[0]); else y_batch<XB, LIM, YD>(B, A, yG, gx, Wy, finf, h, ydm[0]);
@@ -344,6 +369,14 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
             __syncthreads();                       // y-swept row complete; raw rows up to r are free
             if (r + XY_NS <= rlast) issue_row(r + XY_NS, stage);
             double carry = 0.0;
+            if constexpr (VL_XY_OWN && XB == CH && XD != 0) {
+                double o[XB];
+                x_chunk_own<XB, LIM, XD, 1>(h, o, sh, ix0, nx, X8, cofs, Wx, finf);
+                if (store) {
+#pragma unroll
+                    for (int i = 0; i < XB; ++i) __stcs(po + (long)(XD > 0 ? i : XB - 1 - i) * S, o[i]);
+                }
+            } else {
 #pragma unroll
             for (int k = 0; k < XB / CH; ++k) {
                 double o[CH];
@@ -360,6 +393,7 @@ __global__ void __launch_bounds__(VL_XY_MAXT, VL_XY_MINB) sweep_xy_kernel(const 
                         for (int i = 0; i < CH; ++i) __stcs(po + (long)(XB - 1 - (k * CH + i)) * S, o[i]);
                     }
                 }
+            }
             }
         }
     };
