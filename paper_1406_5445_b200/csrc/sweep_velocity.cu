@@ -18,6 +18,7 @@
 #include <map>
 #include <mutex>
 #include <tuple>
+#include <type_traits>
 #include "vlasov_internal.cuh"
 #include "tma.cuh"
 
@@ -192,6 +193,17 @@ constexpr int V_PAD = 3;
 #ifndef VL_YZ_MINB
 #define VL_YZ_MINB 3
 #endif
+#ifndef VL_LITE_PEEL
+#define VL_LITE_PEEL 1
+#endif
+// faces per trip of the lite walk's rolled loop: 4 for the 32x32 vy+vz kernel (2.90 -> 2.85 ms per cycle of config 3), 2
+// elsewhere (4 measured 5 % slower on 48x48 planes, 8 misses the instruction cache: 1.41 -> 1.62 ms on nv32)
+#ifndef VL_LITE_UNROLL
+#define VL_LITE_UNROLL 2
+#endif
+#ifndef VL_LITE_UNROLL32
+#define VL_LITE_UNROLL32 4
+#endif
 
 struct OutShared {       // cells of a line in shared memory: cell0 = byte address of cell a
     unsigned a; int st8;
@@ -319,7 +331,7 @@ __device__ __forceinline__ void march_seg_small(unsigned L, int st8, int N, int 
 // whole-cell sums nor the cell itself.  A face against the flow (CROSS, n = 0 there) reads its foot one cell downstream,
 // mirrored, and its own cell is fp.  The last face of the box carries no flux (R7): its S is added back, cell by cell.
 //   flow cell c <-> cell a+c (sigma >= 0) | a+SEG-1-c (sigma < 0);  walk face m lies between flow cells m-1 and m.
-template <int SEG, int LIM, int FULL, int CROSS, class Out>
+template <int SEG, int LIM, int FULL, int CROSS, int LU, class Out>
 __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a, double sig_a, double sig_b,
                                                double s1, double finf, Out out) {
     const double M = 6755399441055744.0;
@@ -333,9 +345,11 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
     out.step(pos ? 1 : -1);
     double Gp = 0.0;
     int np = 0;
-    // three faces per trip of a rolled loop: the walks of a sweep must share the 32 KB instruction cache
-#pragma unroll 3
-    for (int m = 0; m <= SEG; ++m) {
+    // The first face only leaves its flux behind and is peeled off (its special cases cost five predicated instructions
+    // at every face of a rolled loop); the other SEG faces run VL_LITE_UNROLL per trip of a rolled loop: the walks of a
+    // sweep must share the 32 KB instruction cache.
+    auto face = [&](int m, auto first_c) {
+        constexpr bool FIRST = decltype(first_c)::value;
         const double at = fabs(tau);
         const double r = __dadd_rd(at, M);
         const int n = __double2loint(r);
@@ -357,7 +371,7 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
         double c1, c2;
         pfc_weights(bq, c1, c2);
         double G = bs * fma(c1, sp, fma(c2, sm, f0));
-        if (m == 0) {
+        if (FIRST) {
             if (zero_first) G = 0.0;
         } else {
             double T = f0;
@@ -378,14 +392,24 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
         np = n;
         tau += s1;
         fb += u;
-    }
+    };
+#if VL_LITE_PEEL
+    face(0, std::true_type{});
+    constexpr int LITE_UNROLL = LU;
+#pragma unroll LITE_UNROLL
+    for (int m = 1; m <= SEG; ++m) face(m, std::false_type{});
+#else
+#pragma unroll 3
+    for (int m = 0; m <= SEG; ++m) { if (m == 0) face(m, std::true_type{}); else face(m, std::false_type{}); }
+#endif
 }
 
 // One thread remaps cells [a, b) of one line: flux per face, eq. (38) per cell.  sigma of face k is
 // s0 + s1 k (accumulated).  out.put(value) stores the new average of the next cell (a, a+1, ...).
 // FAST: 8-cell segments may take the flow-ordered walks (2: every lane of the warp is here).  LOOSE: the 4th cell
 // before a line is readable memory (any value), which admits floor|sigma| = 2 at a box face.
-template <int LIM, int FAST, int LOOSE = 0, int NB = 1, class Out>
+// LU: faces per trip of the rolled loop of march_seg_lite (after its peeled first face).
+template <int LIM, int FAST, int LOOSE = 0, int NB = 1, int LU = VL_LITE_UNROLL, class Out>
 __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
                                             double finf, Out& out) {
     if (a >= b) return;                              // a trailing work item beyond the end of the line: nothing to do
@@ -410,8 +434,8 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
         const double bound = (LOOSE && dist == 0) ? (double)V_PAD - 0.5 : (double)(min(dist, 32) + V_PAD - 1);
         const bool lite = fabs(t0) < bound && fabs(s1) <= 0.5 && (!cross || sub);
         if (__all_sync(mask, lite)) {
-            if (__any_sync(mask, cross)) march_seg_lite<SEG, LIM, FULL, 1>(L, st8, N, a, sig, sig_b, s1, finf, out);
-            else march_seg_lite<SEG, LIM, FULL, 0>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            if (__any_sync(mask, cross)) march_seg_lite<SEG, LIM, FULL, 1, LU>(L, st8, N, a, sig, sig_b, s1, finf, out);
+            else march_seg_lite<SEG, LIM, FULL, 0, LU>(L, st8, N, a, sig, sig_b, s1, finf, out);
             return;
         }
     }
@@ -829,7 +853,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
                 const int a = seg * seglen, b = a + seglen;          // CN is a multiple of 8: whole segments
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM, FW, 1, VL_YZ_BATCH>(sSt + (unsigned)((SP0 + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH, (CN == 32 ? VL_LITE_UNROLL32 : VL_LITE_UNROLL)>(sSt + (unsigned)((SP0 + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
@@ -844,7 +868,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
                 const int a = seg * seglen, b = a + seglen;
                 OutShared o{smem_addr(A + OFFA + p * PSA + y * RSA + a), 8};
-                march_cells<LIM, FW, 1, VL_YZ_BATCH>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH, (CN == 32 ? VL_LITE_UNROLL32 : VL_LITE_UNROLL)>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
             }
         }
         __syncthreads();                           // vz done: A complete
