@@ -409,7 +409,8 @@ __device__ __forceinline__ void march_seg_lite(unsigned L, int st8, int N, int a
 // FAST: 8-cell segments may take the flow-ordered walks (2: every lane of the warp is here).  LOOSE: the 4th cell
 // before a line is readable memory (any value), which admits floor|sigma| = 2 at a box face.
 // LU: faces per trip of the rolled loop of march_seg_lite (after its peeled first face).
-template <int LIM, int FAST, int LOOSE = 0, int NB = 1, int LU = VL_LITE_UNROLL, class Out>
+// PAD: zero cells on either side of the line (V_PAD, or more where the caller's layout has them).
+template <int LIM, int FAST, int LOOSE = 0, int NB = 1, int LU = VL_LITE_UNROLL, int PAD = V_PAD, class Out>
 __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, int b, double s0, double s1,
                                             double finf, Out& out) {
     if (a >= b) return;                              // a trailing work item beyond the end of the line: nothing to do
@@ -426,12 +427,12 @@ __device__ __forceinline__ void march_cells(unsigned L, int st8, int N, int a, i
             march_seg_small<SEG, LIM, FULL, NB>(L, st8, N, a, sig, sig_b, s1, finf, out);
             return;
         }
-        // march_seg_lite: its first face reads flow cells -3-n .. -1-n, with V_PAD zero cells before the line; the
+        // march_seg_lite: its first face reads flow cells -3-n .. -1-n, with PAD zero cells before the line; the
         // reads of a box face are discarded (zero flux), and n grows by less than 1/2 per face
         const bool pos = !(sig < 0.0 || sig_b < 0.0);
         const double t0 = pos ? sig : sig_b;
         const int dist = pos ? a : N - b;              // cells between the box face and the first face of the walk
-        const double bound = (LOOSE && dist == 0) ? (double)V_PAD - 0.5 : (double)(min(dist, 32) + V_PAD - 1);
+        const double bound = (LOOSE && dist == 0) ? (double)PAD - 0.5 : (double)(min(dist, 32) + PAD - 1);
         const bool lite = fabs(t0) < bound && fabs(s1) <= 0.5 && (!cross || sub);
         if (__all_sync(mask, lite)) {
             if (__any_sync(mask, cross)) march_seg_lite<SEG, LIM, FULL, 1, LU>(L, st8, N, a, sig, sig_b, s1, finf, out);
@@ -754,11 +755,20 @@ __host__ __device__ constexpr int yz_tma_minb(int cn) { return cn == 48 ? VL_YZ4
 #ifndef VL_YZ_COMPACT
 #define VL_YZ_COMPACT 1
 #endif
-__host__ __device__ constexpr int yz_tma_spad(int cn) { return VL_YZ_COMPACT && cn % 16 == 0 ? V_PAD : 8; }
+// Zero cells on either side of a line in this kernel's buffers.  A box-face segment whose lanes reach floor|sigma| =
+// pad falls back to the general face walk, warp and all: at 48^3 the GEM electrons reach 3.2 cells, and a third of the
+// electron warps did (nv48 vy+vz 5.85 -> 4.9 ms per cycle with the walk admitted).  5 for 40x40 and 48x48 planes.
+#ifndef VL_YZ_PAD5
+#define VL_YZ_PAD5 1
+#endif
+__host__ __device__ constexpr int yz_tma_pad(int cn) { return VL_YZ_PAD5 && (cn == 40 || cn == 48) ? 5 : V_PAD; }
+__host__ __device__ constexpr int yz_tma_spad(int cn) { return VL_YZ_COMPACT && cn % 16 == 0 ? yz_tma_pad(cn) : 8; }
 // (the walks may look at the 4th row before a line, whatever it holds: one more row before the first plane)
-__host__ __device__ constexpr int yz_tma_spad0(int cn) { return yz_tma_spad(cn) > V_PAD ? yz_tma_spad(cn) : V_PAD + 1; }
+__host__ __device__ constexpr int yz_tma_spad0(int cn) { return yz_tma_spad(cn) > yz_tma_pad(cn) ? yz_tma_spad(cn) : yz_tma_pad(cn) + 1; }
 __host__ __device__ constexpr int yz_tma_stg(int cn) { return ((yz_tma_spad0(cn) + yz_tma_planes(cn) * (cn + yz_tma_spad(cn))) * cn + 15) & ~15; }
-__host__ __device__ constexpr int yz_tma_buf(int cn) { return (V_PAD * (cn + V_PAD) + V_PAD + yz_tma_planes(cn) * (cn + V_PAD) * (cn + V_PAD) + 1) & ~1; }
+// Bf is read along z only: no pad rows, the rows of all planes follow each other at pitch N2 + pad (odd), the gap is the
+// right pad of one row and the left pad of the next; pad + 1 cells before the first row and after the last.
+__host__ __device__ constexpr int yz_tma_buf(int cn) { return (2 * (yz_tma_pad(cn) + 1) + yz_tma_planes(cn) * cn * (cn + yz_tma_pad(cn)) + 1) & ~1; }
 __host__ __device__ constexpr int yz_tma_rsa(int cn) { return VL_YZ_COMPACT ? (cn | 1) : cn + V_PAD; }
 __host__ __device__ constexpr int yz_tma_psa(int cn) { return VL_YZ_COMPACT ? cn * yz_tma_rsa(cn) : (cn + V_PAD) * (cn + V_PAD); }
 __host__ __device__ constexpr int yz_tma_offa(int cn) { return VL_YZ_COMPACT ? 0 : V_PAD * (cn + V_PAD) + V_PAD; }
@@ -773,8 +783,10 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
     constexpr int N1 = CN, N2 = CN, plane = CN * CN;
     constexpr int ct = yz_tma_planes(CN);
     constexpr int nseg = (CN + 7) / 8, seglen = (CN + nseg - 1) / nseg;
-    constexpr int RS = N2 + V_PAD, PS = (N1 + V_PAD) * RS, OFF = V_PAD * RS + V_PAD;
-    constexpr int BUF = (OFF + ct * PS + 1) & ~1;
+    constexpr int YZP = yz_tma_pad(CN);                          // zero cells on either side of a line
+    constexpr int RS = N2 + YZP, PS = N1 * RS, OFF = YZP + 1;    // Bf: see yz_tma_buf
+    constexpr int BUF = yz_tma_buf(CN);
+    static_assert(RS % 2 == 1 && OFF + ct * PS + YZP + 1 <= BUF, "odd pitch, pads inside the buffer");
     constexpr int SPAD = yz_tma_spad(CN);                        // pad rows of the staging buffer: >= V_PAD, and 8 rows of
                                                                  // any even N2 keep every TMA box 128-byte aligned
     constexpr int SP0 = yz_tma_spad0(CN);                        // rows before the first plane
@@ -853,7 +865,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 const double s0 = ty0 + ty2 * (p0 + p) + ty3 * z;
                 const int a = seg * seglen, b = a + seglen;          // CN is a multiple of 8: whole segments
                 OutShared o{smem_addr(Bf + OFF + p * PS + z + a * RS), RS * 8};
-                march_cells<LIM, FW, 1, VL_YZ_BATCH, (CN == 32 ? VL_LITE_UNROLL32 : VL_LITE_UNROLL)>(sSt + (unsigned)((SP0 + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH, (CN == 32 ? VL_LITE_UNROLL32 : VL_LITE_UNROLL), YZP>(sSt + (unsigned)((SP0 + p * (N1 + SPAD)) * N2 + z) * 8, N2 * 8, N1, a, b, s0, ty1, finfy, o);
             }
         }
         __syncthreads();                           // vy done: Bf complete, staging buffer free
@@ -868,7 +880,7 @@ __global__ void __launch_bounds__(yz_tma_threads(CN), yz_tma_minb(CN)) vsweep_yz
                 const double s0 = tz0 + tz2 * (p0 + p) + tz3 * y;
                 const int a = seg * seglen, b = a + seglen;
                 OutShared o{smem_addr(A + OFFA + p * PSA + y * RSA + a), 8};
-                march_cells<LIM, FW, 1, VL_YZ_BATCH, (CN == 32 ? VL_LITE_UNROLL32 : VL_LITE_UNROLL)>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
+                march_cells<LIM, FW, 1, VL_YZ_BATCH, (CN == 32 ? VL_LITE_UNROLL32 : VL_LITE_UNROLL), YZP>(smem_addr(Bf + OFF + p * PS + y * RS), 8, N2, a, b, s0, tz1, finfz, o);
             }
         }
         __syncthreads();                           // vz done: A complete
